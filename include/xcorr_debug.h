@@ -1,0 +1,40 @@
+/*
+ * xcorr_debug.h -- test-support entry points of libxcorr.so.  NOT part of the product path:
+ * xcorr_process()/xcorr_read() never call any of these and nothing dispatches to them.
+ */
+#ifndef XCORR_DEBUG_H_
+#define XCORR_DEBUG_H_
+
+#include <stdint.h>
+#include "xcorr.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/*
+ * The host-side work decomposition xcorr_create() would build for `n_workers` CTA pairs (no GPU needed).
+ * A work item is a 256 x 256 super-tile (f, I <= J) of the visibility matrix ("computes only upper-triangle
+ * tiles", BASELINE.json:north_star (b)); it is cut along time into stages of xcorr_debug_stage_samples()
+ * samples and the stages are dealt to workers.
+ * Returns the number of segments (>= 0) or XCORR_EINVAL.  With non-NULL outputs writes
+ * segments_out[k][6] = {f, I, J, stage_begin, stage_end, tile} (capacity max_segments) and
+ * worker_begin_out[n_workers + 1].
+ */
+int xcorr_debug_schedule(int n_inputs, int n_freq, int t_per_frame, int n_workers,
+                         int32_t *segments_out, int max_segments, int32_t *worker_begin_out);
+
+/* Time samples per pipeline stage. */
+int xcorr_debug_stage_samples(void);
+
+/*
+ * Same contract as xcorr_process(), computed by a plain one-thread-per-element SIMT loop (no TMA, no
+ * tensor cores).  Used by the GPU tests as an on-device second opinion for whole-matrix comparisons at
+ * sizes where the CPU oracle takes minutes; parity itself is always judged against oracle/.
+ */
+int xcorr_debug_process_simt(xcorr_handle *h, const void *packed_frame_dev, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XCORR_DEBUG_H_ */

@@ -1,0 +1,121 @@
+// schedule.hpp -- host-side work decomposition for the persistent X-engine kernel (pure C++, no CUDA).
+//
+// Work item  = one super-tile (f, I <= J) over the whole frame; it is cut along time into STAGES of
+//              kStageT samples.  A diagonal item (I == J) costs 3 MMAs per 32-sample K-step, an
+//              off-diagonal one 4.
+// Worker     = one CTA pair (two SMs, one 2-CTA tcgen05 MMA stream); there are `n_workers` of them.
+//
+// Hybrid data-parallel / stream-K split (integer addition is exact and order independent, so a
+// super-tile may be summed by several workers, each adding its partial into the accumulator):
+//   * the first floor(n_items / n_workers) * n_workers items go round-robin, whole, to the workers --
+//     consecutive items (same channel, neighbouring super-tiles) run at the same time on different
+//     workers, so blocks shared between them are served by L2;
+//   * the stages of the remaining items are dealt out as contiguous runs so that every worker ends
+//     with (nearly) the same total cost ("water filling").
+// Every (item, stage) is assigned to exactly one worker (checked by tests/test_host_logic.py).
+#pragma once
+#include <algorithm>
+#include <cstdint>
+#include <vector>
+
+namespace xc {
+
+constexpr int kStageT = 64;  // time samples per pipeline stage (2 MMA K-steps of 32)
+
+struct Segment {          // 32 bytes, read by the kernel
+    int32_t f;            // channel
+    int32_t I, J;         // super-block row / column (I <= J)
+    int32_t stage_begin;  // [stage_begin, stage_end) in units of kStageT samples
+    int32_t stage_end;
+    int32_t tile;         // f * n_supertiles + supertile_index(I, J)  (accumulator tile)
+    int32_t pad0, pad1;
+};
+
+struct Schedule {
+    int n_workers = 0;
+    int n_stages = 0;                 // stages per item = ceil(T / kStageT)
+    std::vector<Segment> segments;    // grouped by worker
+    std::vector<int32_t> worker_begin;  // size n_workers + 1, offsets into segments
+};
+
+inline Schedule make_schedule(int n_inputs, int n_freq, int n_time, int n_workers)
+{
+    Schedule s;
+    s.n_workers = n_workers;
+    s.n_stages = (n_time + kStageT - 1) / kStageT;
+    const int nb = (n_inputs + 255) / 256;
+    const int nst = nb * (nb + 1) / 2;
+
+    struct Item { int f, I, J, tile; int64_t cost_per_stage; };
+    std::vector<Item> items;
+    items.reserve((size_t)n_freq * nst);
+    for (int f = 0; f < n_freq; ++f)
+        for (int I = 0; I < nb; ++I)
+            for (int J = I; J < nb; ++J)
+                items.push_back({f, I, J, f * nst + (I * (2 * nb - I + 1) / 2 + (J - I)), I == J ? 3 : 4});
+
+    const int64_t n_items = (int64_t)items.size();
+    const int64_t n_dp = (n_items / n_workers) * n_workers;
+    std::vector<std::vector<Segment>> per(n_workers);
+    std::vector<int64_t> load(n_workers, 0);
+
+    for (int64_t u = 0; u < n_dp; ++u) {
+        const Item &it = items[u];
+        const int w = (int)(u % n_workers);
+        per[w].push_back({it.f, it.I, it.J, 0, s.n_stages, it.tile, 0, 0});
+        load[w] += it.cost_per_stage * s.n_stages;
+    }
+
+    // remainder: water-fill
+    int64_t rem_cost = 0;
+    for (int64_t u = n_dp; u < n_items; ++u) rem_cost += items[u].cost_per_stage * s.n_stages;
+    if (rem_cost > 0) {
+        // level L with sum_w max(0, L - load[w]) == rem_cost  (bisection on integers, then exact shares)
+        int64_t lo = *std::min_element(load.begin(), load.end());
+        int64_t hi = *std::max_element(load.begin(), load.end()) + rem_cost;
+        while (lo < hi) {
+            const int64_t mid = lo + (hi - lo) / 2;
+            int64_t cap = 0;
+            for (int w = 0; w < n_workers; ++w) cap += std::max<int64_t>(0, mid - load[w]);
+            if (cap >= rem_cost) hi = mid; else lo = mid + 1;
+        }
+        std::vector<int64_t> share(n_workers);
+        int64_t total = 0;
+        for (int w = 0; w < n_workers; ++w) { share[w] = std::max<int64_t>(0, lo - load[w]); total += share[w]; }
+        // trim the surplus (total >= rem_cost) from the last workers with a share
+        for (int w = n_workers - 1; w >= 0 && total > rem_cost; --w) {
+            const int64_t cut = std::min(share[w], total - rem_cost);
+            share[w] -= cut; total -= cut;
+        }
+        // walk the remaining stages in order, handing out contiguous runs
+        int w = 0;
+        int64_t boundary = share[0];  // cumulative cost position where worker w's run ends
+        int64_t pos = 0;
+        for (int64_t u = n_dp; u < n_items; ++u) {
+            const Item &it = items[u];
+            int st = 0;
+            while (st < s.n_stages) {
+                while (w < n_workers - 1 && pos >= boundary) { ++w; boundary += share[w]; }
+                // stages of this item that start before `boundary`
+                int64_t room = boundary - pos;
+                int take = (w == n_workers - 1) ? (s.n_stages - st)
+                                                : (int)std::min<int64_t>(s.n_stages - st, (room + it.cost_per_stage - 1) / it.cost_per_stage);
+                if (take <= 0) take = 1;
+                per[w].push_back({it.f, it.I, it.J, st, st + take, it.tile, 0, 0});
+                load[w] += it.cost_per_stage * take;
+                pos += it.cost_per_stage * take;
+                st += take;
+            }
+        }
+    }
+
+    s.worker_begin.resize(n_workers + 1);
+    for (int w = 0; w < n_workers; ++w) {
+        s.worker_begin[w] = (int32_t)s.segments.size();
+        s.segments.insert(s.segments.end(), per[w].begin(), per[w].end());
+    }
+    s.worker_begin[n_workers] = (int32_t)s.segments.size();
+    return s;
+}
+
+}  // namespace xc

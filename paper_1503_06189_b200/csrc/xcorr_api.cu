@@ -1,0 +1,347 @@
+// xcorr_api.cu -- the C ABI declared in include/xcorr.h: handle management, work schedule, launches.
+// All arithmetic of the hot path runs in the kernels of xengine_kernel.cuh / finalize_kernel.cuh.
+#include "../../include/xcorr.h"
+#include "../../include/xcorr_debug.h"
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "finalize_kernel.cuh"
+#include "layout.hpp"
+#include "schedule.hpp"
+#include "xengine_kernel.cuh"
+
+using namespace xc;
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                    const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct xcorr_handle {
+    int n_inputs = 0, n_freq = 0, n_time = 0;
+    int device = 0;
+    int n_workers = 0;
+    int n_tiles = 0;                 // F * n_supertiles
+    bool offdiag = false;            // N > 256: kernel variant with the column block and -Im plane
+    size_t frame_bytes = 0, output_bytes = 0, acc_bytes = 0;
+    int32_t *acc = nullptr;          // device accumulator (layout.hpp)
+    int32_t *staging = nullptr;      // device packed triangle for host reads
+    Segment *segments = nullptr;     // device
+    int32_t *worker_begin = nullptr; // device
+    long long samples_since_read = 0;
+    uint64_t launches = 0;
+    int last_cuda_error = 0;
+    PFN_encodeTiled encode = nullptr;
+};
+
+struct xcorr_stream {
+    xcorr_handle *h = nullptr;
+    int depth = 0;
+    uint8_t *buf[8] = {};
+    cudaEvent_t copied[8] = {}, consumed[8] = {};
+    cudaStream_t copy_stream = nullptr, compute_stream = nullptr;
+    unsigned long long submitted = 0;
+};
+
+#define XC_CUDA(h, expr)                                  \
+    do {                                                  \
+        cudaError_t e_ = (expr);                          \
+        if (e_ != cudaSuccess) {                          \
+            if (h) (h)->last_cuda_error = (int)e_;        \
+            return e_ == cudaErrorMemoryAllocation ? XCORR_ENOMEM : XCORR_ECUDA; \
+        }                                                 \
+    } while (0)
+
+extern "C" const char *xcorr_strerror(int code)
+{
+    switch (code) {
+        case XCORR_OK: return "ok";
+        case XCORR_EINVAL: return "invalid argument";
+        case XCORR_EARCH: return "current CUDA device is not compute capability 10.x (B200, sm_100a)";
+        case XCORR_ENOMEM: return "out of memory";
+        case XCORR_ECUDA: return "CUDA call failed (see xcorr_last_cuda_error)";
+        case XCORR_EOVERFLOW: return "integration too long: an int32 visibility could overflow";
+        default: return "unknown xcorr error code";
+    }
+}
+
+extern "C" int xcorr_last_cuda_error(const xcorr_handle *h) { return h ? h->last_cuda_error : 0; }
+extern "C" size_t xcorr_frame_bytes(const xcorr_handle *h) { return h ? h->frame_bytes : 0; }
+extern "C" size_t xcorr_output_bytes(const xcorr_handle *h) { return h ? h->output_bytes : 0; }
+extern "C" uint64_t xcorr_kernel_launches(const xcorr_handle *h) { return h ? h->launches : 0; }
+
+static int validate_shape(int n_inputs, int n_freq, int t_per_frame)
+{
+    if (n_inputs <= 0 || n_freq <= 0 || t_per_frame <= 0) return XCORR_EINVAL;
+    if (n_inputs % 16 != 0) return XCORR_EINVAL;
+    if (n_inputs > 65536 || n_freq > 65535) return XCORR_EINVAL;
+    const unsigned long long bytes = (unsigned long long)n_inputs * (unsigned long long)n_freq * (unsigned long long)t_per_frame;
+    if (bytes > (1ull << 40)) return XCORR_EINVAL;
+    return XCORR_OK;
+}
+
+extern "C" void xcorr_destroy(xcorr_handle *h)
+{
+    if (!h) return;
+    cudaSetDevice(h->device);
+    cudaDeviceSynchronize();
+    cudaFree(h->acc);
+    cudaFree(h->staging);
+    cudaFree(h->segments);
+    cudaFree(h->worker_begin);
+    delete h;
+}
+
+extern "C" int xcorr_create(int n_inputs, int n_freq, int t_per_frame, xcorr_handle **out)
+{
+    if (!out) return XCORR_EINVAL;
+    *out = nullptr;
+    int rc = validate_shape(n_inputs, n_freq, t_per_frame);
+    if (rc != XCORR_OK) return rc;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return XCORR_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return XCORR_ECUDA;
+    if (prop.major != 10) return XCORR_EARCH;
+
+    xcorr_handle *h = new (std::nothrow) xcorr_handle;
+    if (!h) return XCORR_ENOMEM;
+    h->n_inputs = n_inputs;
+    h->n_freq = n_freq;
+    h->n_time = t_per_frame;
+    h->device = dev;
+    h->frame_bytes = (size_t)n_inputs * n_freq * t_per_frame;
+    h->output_bytes = (size_t)n_freq * ((size_t)n_inputs * (n_inputs + 1) / 2) * 8;
+    const int nb = n_super(n_inputs);
+    h->n_tiles = n_freq * n_supertiles(nb);
+    h->acc_bytes = (size_t)h->n_tiles * kAccElemsPerTile * sizeof(int32_t);
+    h->offdiag = nb > 1;
+    h->n_workers = prop.multiProcessorCount / 2;
+    if (h->n_workers < 1) { delete h; return XCORR_EARCH; }
+
+    auto fail = [&](int code) { xcorr_destroy(h); return code; };
+
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return fail(XCORR_ECUDA);
+    h->encode = (PFN_encodeTiled)fn;
+
+    const Schedule sched = make_schedule(n_inputs, n_freq, t_per_frame, h->n_workers);
+    cudaError_t e;
+    if ((e = cudaMalloc(&h->acc, h->acc_bytes)) != cudaSuccess) { h->last_cuda_error = e; return fail(XCORR_ENOMEM); }
+    if ((e = cudaMalloc(&h->staging, h->output_bytes)) != cudaSuccess) { h->last_cuda_error = e; return fail(XCORR_ENOMEM); }
+    if ((e = cudaMalloc(&h->segments, sizeof(Segment) * (sched.segments.size() + 1))) != cudaSuccess) return fail(XCORR_ENOMEM);
+    if ((e = cudaMalloc(&h->worker_begin, sizeof(int32_t) * sched.worker_begin.size())) != cudaSuccess) return fail(XCORR_ENOMEM);
+    if (cudaMemset(h->acc, 0, h->acc_bytes) != cudaSuccess) return fail(XCORR_ECUDA);
+    if (!sched.segments.empty() &&
+        cudaMemcpy(h->segments, sched.segments.data(), sizeof(Segment) * sched.segments.size(), cudaMemcpyHostToDevice) != cudaSuccess)
+        return fail(XCORR_ECUDA);
+    if (cudaMemcpy(h->worker_begin, sched.worker_begin.data(), sizeof(int32_t) * sched.worker_begin.size(), cudaMemcpyHostToDevice) !=
+        cudaSuccess)
+        return fail(XCORR_ECUDA);
+
+    if (h->offdiag)
+        e = cudaFuncSetAttribute(xengine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, KernelCfg<true>::kSmemBytes);
+    else
+        e = cudaFuncSetAttribute(xengine_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, KernelCfg<false>::kSmemBytes);
+    if (e != cudaSuccess) { h->last_cuda_error = e; return fail(XCORR_ECUDA); }
+    if (cudaDeviceSynchronize() != cudaSuccess) return fail(XCORR_ECUDA);
+    *out = h;
+    return XCORR_OK;
+}
+
+static int encode_frame_map(xcorr_handle *h, const void *frame_dev, CUtensorMap *map)
+{
+    // a1: global uint8[T][F][N] seen as a 3-D tensor (n, f, t); one box = 128 inputs x 1 channel x kStageT samples,
+    // written to smem as kStageT rows of 128 bytes with the 128-byte swizzle the MMA descriptors expect.
+    const cuuint64_t dims[3] = {(cuuint64_t)h->n_inputs, (cuuint64_t)h->n_freq, (cuuint64_t)h->n_time};
+    const cuuint64_t strides[2] = {(cuuint64_t)h->n_inputs, (cuuint64_t)h->n_inputs * (cuuint64_t)h->n_freq};
+    const cuuint32_t box[3] = {(cuuint32_t)kBlock, 1u, (cuuint32_t)kStageT};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void *>(frame_dev), dims, strides, box, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        h->last_cuda_error = (int)r;
+        return XCORR_ECUDA;
+    }
+    return XCORR_OK;
+}
+
+static int check_process_args(xcorr_handle *h, const void *frame)
+{
+    if (!h || !frame) return XCORR_EINVAL;
+    if (((uintptr_t)frame & 15u) != 0) return XCORR_EINVAL;
+    // |sum| <= 128 * samples must stay <= 2^31 - 1
+    if (h->samples_since_read + (long long)h->n_time > 16777215ll) return XCORR_EOVERFLOW;
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void *cuda_stream)
+{
+    int rc = check_process_args(h, packed_frame_dev);
+    if (rc != XCORR_OK) return rc;
+    alignas(64) CUtensorMap map;
+    rc = encode_frame_map(h, packed_frame_dev, &map);
+    if (rc != XCORR_OK) return rc;
+    KernelParams p;
+    p.segments = h->segments;
+    p.worker_begin = h->worker_begin;
+    p.acc = h->acc;
+    p.n_inputs = h->n_inputs;
+    p.n_freq = h->n_freq;
+    p.n_time = h->n_time;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const dim3 grid(2 * h->n_workers), block(kThreads);
+    if (h->offdiag)
+        xengine_kernel<true><<<grid, block, KernelCfg<true>::kSmemBytes, s>>>(map, p);
+    else
+        xengine_kernel<false><<<grid, block, KernelCfg<false>::kSmemBytes, s>>>(map, p);
+    XC_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    h->samples_since_read += h->n_time;
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_read(xcorr_handle *h, int32_t *upper_triangle_out, void *cuda_stream)
+{
+    if (!h || !upper_triangle_out) return XCORR_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaPointerAttributes attr;
+    bool on_device = false;
+    if (cudaPointerGetAttributes(&attr, upper_triangle_out) == cudaSuccess)
+        on_device = (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged);
+    else
+        cudaGetLastError();
+    if (on_device && ((uintptr_t)upper_triangle_out & 15u) != 0) return XCORR_EINVAL;
+    int32_t *dst = on_device ? upper_triangle_out : h->staging;
+    const int nt = (h->n_inputs + 31) / 32;
+    finalize_kernel<<<dim3(nt, nt, h->n_freq), dim3(32, 8), 0, s>>>(h->acc, dst, h->n_inputs);
+    XC_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, s));      // ends the integration
+    h->samples_since_read = 0;
+    if (!on_device) {
+        XC_CUDA(h, cudaMemcpyAsync(upper_triangle_out, h->staging, h->output_bytes, cudaMemcpyDeviceToHost, s));
+        XC_CUDA(h, cudaStreamSynchronize(s));
+    }
+    return XCORR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// streamed frame path (a5)
+// ---------------------------------------------------------------------------------------------------
+extern "C" void xcorr_stream_destroy(xcorr_stream *s)
+{
+    if (!s) return;
+    if (s->h) cudaSetDevice(s->h->device);
+    cudaDeviceSynchronize();
+    for (int k = 0; k < s->depth; ++k) {
+        if (s->buf[k]) cudaFree(s->buf[k]);
+        if (s->copied[k]) cudaEventDestroy(s->copied[k]);
+        if (s->consumed[k]) cudaEventDestroy(s->consumed[k]);
+    }
+    if (s->copy_stream) cudaStreamDestroy(s->copy_stream);
+    if (s->compute_stream) cudaStreamDestroy(s->compute_stream);
+    delete s;
+}
+
+extern "C" int xcorr_stream_create(xcorr_handle *h, int depth, xcorr_stream **out)
+{
+    if (!h || !out || depth < 2 || depth > 8) return XCORR_EINVAL;
+    *out = nullptr;
+    xcorr_stream *s = new (std::nothrow) xcorr_stream;
+    if (!s) return XCORR_ENOMEM;
+    s->h = h;
+    s->depth = depth;
+    auto fail = [&](int code) { xcorr_stream_destroy(s); return code; };
+    if (cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(XCORR_ECUDA);
+    if (cudaStreamCreateWithFlags(&s->compute_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(XCORR_ECUDA);
+    for (int k = 0; k < depth; ++k) {
+        if (cudaMalloc(&s->buf[k], h->frame_bytes) != cudaSuccess) return fail(XCORR_ENOMEM);
+        if (cudaEventCreateWithFlags(&s->copied[k], cudaEventDisableTiming) != cudaSuccess) return fail(XCORR_ECUDA);
+        if (cudaEventCreateWithFlags(&s->consumed[k], cudaEventDisableTiming) != cudaSuccess) return fail(XCORR_ECUDA);
+    }
+    *out = s;
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_stream_submit(xcorr_stream *s, const void *frame_host)
+{
+    if (!s || !frame_host) return XCORR_EINVAL;
+    xcorr_handle *h = s->h;
+    if (h->samples_since_read + (long long)h->n_time > 16777215ll) return XCORR_EOVERFLOW;
+    const int k = (int)(s->submitted % (unsigned long long)s->depth);
+    if (s->submitted >= (unsigned long long)s->depth) {
+        // ring-buffer back-pressure: the correlation that last read this device buffer must have finished
+        XC_CUDA(h, cudaEventSynchronize(s->consumed[k]));
+    }
+    XC_CUDA(h, cudaMemcpyAsync(s->buf[k], frame_host, h->frame_bytes, cudaMemcpyHostToDevice, s->copy_stream));
+    XC_CUDA(h, cudaEventRecord(s->copied[k], s->copy_stream));
+    XC_CUDA(h, cudaStreamWaitEvent(s->compute_stream, s->copied[k], 0));
+    const int rc = xcorr_process(h, s->buf[k], (void *)s->compute_stream);
+    if (rc != XCORR_OK) return rc;
+    XC_CUDA(h, cudaEventRecord(s->consumed[k], s->compute_stream));
+    s->submitted += 1;
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_stream_sync(xcorr_stream *s)
+{
+    if (!s) return XCORR_EINVAL;
+    XC_CUDA(s->h, cudaStreamSynchronize(s->copy_stream));
+    XC_CUDA(s->h, cudaStreamSynchronize(s->compute_stream));
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_stream_read(xcorr_stream *s, int32_t *upper_triangle_out)
+{
+    if (!s || !upper_triangle_out) return XCORR_EINVAL;
+    const int rc = xcorr_read(s->h, upper_triangle_out, (void *)s->compute_stream);
+    if (rc != XCORR_OK) return rc;
+    XC_CUDA(s->h, cudaStreamSynchronize(s->compute_stream));
+    return XCORR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// debug / test support (include/xcorr_debug.h) -- never on the xcorr_process path
+// ---------------------------------------------------------------------------------------------------
+extern "C" int xcorr_debug_schedule(int n_inputs, int n_freq, int t_per_frame, int n_workers, int32_t *segments_out, int max_segments,
+                                    int32_t *worker_begin_out)
+{
+    if (validate_shape(n_inputs, n_freq, t_per_frame) != XCORR_OK || n_workers <= 0) return XCORR_EINVAL;
+    const Schedule sched = make_schedule(n_inputs, n_freq, t_per_frame, n_workers);
+    const int n = (int)sched.segments.size();
+    if (segments_out && worker_begin_out) {
+        if (n > max_segments) return XCORR_EINVAL;
+        for (int k = 0; k < n; ++k) {
+            const Segment &g = sched.segments[k];
+            int32_t *o = segments_out + 6 * k;
+            o[0] = g.f; o[1] = g.I; o[2] = g.J; o[3] = g.stage_begin; o[4] = g.stage_end; o[5] = g.tile;
+        }
+        for (int w = 0; w <= n_workers; ++w) worker_begin_out[w] = sched.worker_begin[w];
+    }
+    return n;
+}
+
+extern "C" int xcorr_debug_stage_samples(void) { return kStageT; }
+
+extern "C" int xcorr_debug_process_simt(xcorr_handle *h, const void *packed_frame_dev, void *cuda_stream)
+{
+    int rc = check_process_args(h, packed_frame_dev);
+    if (rc != XCORR_OK) return rc;
+    const int blocks = h->n_tiles * 2 * (kBlock / 8);
+    simt_reference_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const uint8_t *)packed_frame_dev, h->acc, h->n_inputs,
+                                                                            h->n_freq, h->n_time);
+    XC_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    h->samples_since_read += h->n_time;
+    return XCORR_OK;
+}

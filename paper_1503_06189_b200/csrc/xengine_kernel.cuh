@@ -1,0 +1,307 @@
+// xengine_kernel.cuh -- the fused X-engine kernel for sm_100a (hot-path rows a1..a4).
+//
+//   a1  TMA stages packed bytes  frame[t][f][128 inputs]  as 128-byte rows (SWIZZLE_128B) into smem
+//   a2  unpack warps split each byte into int8 Re / Im planes (same swizzled 128-byte-row layout, so
+//       the unpack is purely element-wise and never looks at the swizzle)
+//   a3  one thread issues 2-CTA tcgen05.mma kind::i8 (M = 256 over the CTA pair, N = 256, K = 32) with
+//       both operands MN-major straight from those planes; int32 accumulators stay in TMEM (512 columns)
+//       for the whole time range of the work segment
+//   a4  epilogue warps tcgen05.ld the accumulators and red.add them into the device accumulator
+//
+// Complex product from stacked real GEMMs (BASELINE.json:north_star (b)); h = Re plane, l = Im plane:
+//   diagonal super-tile (I == J):   R += h h^T ; R += l l^T ; Q += l h^T      (Im V = Q - Q^T, formed at read)
+//   off-diagonal        (I <  J):   R += h_I h_J^T ; R += l_I l_J^T ; Q += l_I h_J^T ; Q += h_I (-l_J)^T
+// Integer MMAs have no operand-negate bit, hence the explicit -l_J plane for I < J.
+//
+// One cluster = CTA pair = one "worker" of schedule.hpp; CTA rank r owns inputs [128r, 128r+128) of the
+// row super-block (A operand, TMEM lanes) and of the column super-block (its half of the B operand).
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "layout.hpp"
+#include "ptx.cuh"
+#include "schedule.hpp"
+
+namespace xc {
+
+// ------------------------------------------------------------------------------------------------
+// compile-time configuration
+// ------------------------------------------------------------------------------------------------
+template <bool kOffDiag>
+struct KernelCfg {
+    static constexpr int kRowBytes = 128;                          // one t-row of one 128-input block
+    static constexpr int kPlaneBytes = kStageT * kRowBytes;        // 8 KiB: one plane (or packed block) per stage
+    static constexpr int kPackedBlocks = kOffDiag ? 2 : 1;         // A block (+ B block when I < J)
+    static constexpr int kPlanes = kOffDiag ? 5 : 2;               // h_a l_a [h_b l_b -l_b]
+    static constexpr int kPackedStageBytes = kPackedBlocks * kPlaneBytes;
+    static constexpr int kPlaneStageBytes = kPlanes * kPlaneBytes;
+    static constexpr int kPackedStages = kOffDiag ? 3 : 4;
+    static constexpr int kPlaneStages = kOffDiag ? 3 : 6;
+    static constexpr int kSmemData = kPackedStages * kPackedStageBytes + kPlaneStages * kPlaneStageBytes;
+    static constexpr int kSmemBytes = kSmemData + 1024 /*align slack*/ + 1024 /*barriers*/;
+};
+
+constexpr int kThreads = 384;          // 12 warps
+constexpr int kWarpTma = 0;
+constexpr int kWarpMma = 1;
+constexpr int kWarpTmem = 2;
+constexpr int kWarpUnpack0 = 4;        // warps 4..7
+constexpr int kNumUnpackWarps = 4;
+constexpr int kWarpEpi0 = 8;           // warps 8..11 (warp % 4 == TMEM lane quarter)
+constexpr int kNumEpiWarps = 4;
+
+struct KernelParams {
+    const Segment *segments;       // device
+    const int32_t *worker_begin;   // device, n_workers + 1
+    int32_t *acc;                  // device accumulator, layout.hpp
+    int n_inputs;
+    int n_freq;
+    int n_time;
+};
+
+// ------------------------------------------------------------------------------------------------
+// a2: nibble unpack, 4 samples per 32-bit word.  Re = sext4(b >> 4), Im = sext4(b & 15)  (R2, R3)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t unpack_re4(uint32_t w)
+{
+    uint32_t sign;                                               // each byte -> 0xFF if its bit 7 is set else 0x00
+    asm("prmt.b32 %0, %1, %1, 0xBA98;" : "=r"(sign) : "r"(w));    // (selector bit 3 = replicate the byte's sign; __byte_perm masks it off)
+    return ((w >> 4) & 0x0F0F0F0Fu) | (sign & 0xF0F0F0F0u);
+}
+__device__ __forceinline__ uint32_t unpack_im4(uint32_t w)
+{
+    const uint32_t sign = (w & 0x08080808u) * 0x1Eu;             // 0x08 -> 0xF0 inside each byte, no carries
+    return (w & 0x0F0F0F0Fu) | sign;
+}
+// per-byte two's-complement negation of values in [-8, 7] (result in [-7, 8], fits int8)
+__device__ __forceinline__ uint32_t negate4(uint32_t y)
+{
+    return (0x80808080u - (y & 0x7F7F7F7Fu)) ^ (~y & 0x80808080u);
+}
+
+// ------------------------------------------------------------------------------------------------
+// the kernel
+// ------------------------------------------------------------------------------------------------
+template <bool kOffDiag>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams p)
+{
+    using Cfg = KernelCfg<kOffDiag>;
+    extern __shared__ uint8_t smem_raw[];
+
+    const uint32_t warp = threadIdx.x >> 5;
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t rank = ptx::cluster_ctarank();          // 0 = leader (issues the MMAs)
+    const uint32_t worker = blockIdx.x >> 1;
+
+    // ---- shared memory carve-up (1024-byte aligned data, then barriers) ----
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t smem_packed = smem_base;
+    const uint32_t smem_planes = smem_packed + Cfg::kPackedStages * Cfg::kPackedStageBytes;
+    const uint32_t bar_base = smem_planes + Cfg::kPlaneStages * Cfg::kPlaneStageBytes;
+    // barrier slots (8 bytes each)
+    auto bar_pk_full = [&](int s) { return bar_base + 8u * (uint32_t)s; };
+    auto bar_pk_empty = [&](int s) { return bar_base + 8u * (uint32_t)(Cfg::kPackedStages + s); };
+    auto bar_pl_full = [&](int s) { return bar_base + 8u * (uint32_t)(2 * Cfg::kPackedStages + s); };
+    auto bar_pl_empty = [&](int s) { return bar_base + 8u * (uint32_t)(2 * Cfg::kPackedStages + Cfg::kPlaneStages + s); };
+    const uint32_t bar_acc_full = bar_base + 8u * (uint32_t)(2 * Cfg::kPackedStages + 2 * Cfg::kPlaneStages);
+    const uint32_t bar_acc_empty = bar_acc_full + 8u;
+    const uint32_t tmem_slot = bar_acc_empty + 8u;   // uint32 written by tcgen05.alloc
+
+    if (warp == kWarpMma && lane == 0) {
+        for (int s = 0; s < Cfg::kPackedStages; ++s) {
+            ptx::mbar_init(bar_pk_full(s), 1);                    // TMA producer's arrive.expect_tx
+            ptx::mbar_init(bar_pk_empty(s), kNumUnpackWarps);     // one arrive per unpack warp
+        }
+        for (int s = 0; s < Cfg::kPlaneStages; ++s) {
+            ptx::mbar_init(bar_pl_full(s), 2 * kNumUnpackWarps);  // unpack warps of BOTH CTAs (used in the leader only)
+            ptx::mbar_init(bar_pl_empty(s), 1);                   // tcgen05.commit (multicast to both CTAs)
+        }
+        ptx::mbar_init(bar_acc_full, 1);                          // tcgen05.commit (multicast)
+        ptx::mbar_init(bar_acc_empty, 2 * kNumEpiWarps);          // epilogue warps of BOTH CTAs (leader only)
+        ptx::fence_mbar_init();
+    }
+    if (warp == kWarpTma && lane == 0) ptx::prefetch_tensormap(&frame_map);
+    if (warp == kWarpTmem) {
+        ptx::tmem_alloc<2>(tmem_slot, kAccCols);
+        ptx::tmem_relinquish<2>();
+    }
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::cluster_sync();           // barriers of both CTAs initialised before any remote arrive / multicast commit
+    ptx::tc_fence_after_sync();
+
+    uint32_t tmem_base;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+    const int seg_begin = p.worker_begin[worker];
+    const int seg_end = p.worker_begin[worker + 1];
+
+    if (warp == kWarpTma) {
+        // ===================================================== a1: TMA producer (one lane)
+        if (lane == 0) {
+            uint32_t it = 0;
+            for (int sg = seg_begin; sg < seg_end; ++sg) {
+                const Segment seg = p.segments[sg];
+                const int n_a = seg.I * kSuper + (int)rank * kBlock;
+                const int n_b = seg.J * kSuper + (int)rank * kBlock;
+                for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
+                    const uint32_t slot = it % Cfg::kPackedStages;
+                    const uint32_t ph = (it / Cfg::kPackedStages) & 1u;
+                    ptx::mbar_wait(bar_pk_empty(slot), ph ^ 1u);
+                    const uint32_t dst = smem_packed + slot * Cfg::kPackedStageBytes;
+                    const bool off = kOffDiag && (seg.I != seg.J);
+                    ptx::mbar_arrive_expect_tx(bar_pk_full(slot), off ? 2 * Cfg::kPlaneBytes : Cfg::kPlaneBytes);
+                    ptx::tma_load_3d(dst, &frame_map, bar_pk_full(slot), n_a, seg.f, st * kStageT);
+                    if (off) ptx::tma_load_3d(dst + Cfg::kPlaneBytes, &frame_map, bar_pk_full(slot), n_b, seg.f, st * kStageT);
+                }
+            }
+        }
+    } else if (warp == kWarpMma) {
+        // ===================================================== a3: MMA issuer (leader CTA, one lane)
+        if (rank == 0 && lane == 0) {
+            constexpr uint32_t idesc = ptx::make_idesc_i8_mnmajor(256, 256);
+            const uint32_t tmem_R = tmem_base;
+            const uint32_t tmem_Q = tmem_base + 256;
+            uint32_t it = 0, unit = 0;
+            for (int sg = seg_begin; sg < seg_end; ++sg, ++unit) {
+                const Segment seg = p.segments[sg];
+                const bool off = kOffDiag && (seg.I != seg.J);
+                ptx::mbar_wait_cluster(bar_acc_empty, (unit & 1u) ^ 1u);     // epilogues of both CTAs drained TMEM
+                ptx::tc_fence_after_sync();
+                for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
+                    const uint32_t slot = it % Cfg::kPlaneStages;
+                    const uint32_t ph = (it / Cfg::kPlaneStages) & 1u;
+                    ptx::mbar_wait_cluster(bar_pl_full(slot), ph);
+                    ptx::tc_fence_after_sync();
+                    const uint32_t pl = smem_planes + slot * Cfg::kPlaneStageBytes;
+#pragma unroll
+                    for (int k = 0; k < kStageT / 32; ++k) {
+                        const uint32_t koff = (uint32_t)k * 32u * Cfg::kRowBytes;
+                        const uint64_t d_ha = ptx::make_smem_desc_mn_sw128(pl + 0 * Cfg::kPlaneBytes + koff, 1024, 1024);
+                        const uint64_t d_la = ptx::make_smem_desc_mn_sw128(pl + 1 * Cfg::kPlaneBytes + koff, 1024, 1024);
+                        const uint32_t acc = (st != seg.stage_begin || k != 0) ? 1u : 0u;
+                        if (!off) {
+                            ptx::mma_i8<2>(tmem_R, d_ha, d_ha, idesc, acc);   // R  = h h^T
+                            ptx::mma_i8<2>(tmem_R, d_la, d_la, idesc, 1u);    // R += l l^T
+                            ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc, acc);   // Q  = l h^T
+                        } else {
+                            const uint64_t d_hb = ptx::make_smem_desc_mn_sw128(pl + 2 * Cfg::kPlaneBytes + koff, 1024, 1024);
+                            const uint64_t d_lb = ptx::make_smem_desc_mn_sw128(pl + 3 * Cfg::kPlaneBytes + koff, 1024, 1024);
+                            const uint64_t d_nb = ptx::make_smem_desc_mn_sw128(pl + 4 * Cfg::kPlaneBytes + koff, 1024, 1024);
+                            ptx::mma_i8<2>(tmem_R, d_ha, d_hb, idesc, acc);   // R  = h_I h_J^T
+                            ptx::mma_i8<2>(tmem_R, d_la, d_lb, idesc, 1u);    // R += l_I l_J^T
+                            ptx::mma_i8<2>(tmem_Q, d_la, d_hb, idesc, acc);   // Q  = l_I h_J^T
+                            ptx::mma_i8<2>(tmem_Q, d_ha, d_nb, idesc, 1u);    // Q += h_I (-l_J)^T
+                        }
+                    }
+                    ptx::mma_commit<2>(bar_pl_empty(slot), 0x3);   // planes of this stage may be overwritten (both CTAs)
+                }
+                ptx::mma_commit<2>(bar_acc_full, 0x3);             // accumulators complete (both CTAs)
+            }
+        }
+    } else if (warp >= kWarpUnpack0 && warp < kWarpUnpack0 + kNumUnpackWarps) {
+        // ===================================================== a2: unpack warps
+        const uint32_t tid = threadIdx.x - kWarpUnpack0 * 32;     // 0..127
+        const uint32_t pl_full_leader = ptx::mapa(bar_base, 0) + (bar_pl_full(0) - bar_base);
+        uint32_t it = 0;
+        for (int sg = seg_begin; sg < seg_end; ++sg) {
+            const Segment seg = p.segments[sg];
+            const bool off = kOffDiag && (seg.I != seg.J);
+            for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
+                const uint32_t pslot = it % Cfg::kPackedStages, pph = (it / Cfg::kPackedStages) & 1u;
+                const uint32_t lslot = it % Cfg::kPlaneStages, lph = (it / Cfg::kPlaneStages) & 1u;
+                ptx::mbar_wait(bar_pk_full(pslot), pph);                      // TMA bytes landed
+                ptx::mbar_wait_cluster(bar_pl_empty(lslot), lph ^ 1u);        // MMAs that read this plane slot retired
+                const uint32_t src = smem_packed + pslot * Cfg::kPackedStageBytes;
+                const uint32_t dst = smem_planes + lslot * Cfg::kPlaneStageBytes;
+#pragma unroll
+                for (int q = 0; q < Cfg::kPlaneBytes / (128 * 16); ++q) {
+                    const uint32_t o = (uint32_t)(q * 128 + tid) * 16u;
+                    uint32_t w0, w1, w2, w3;
+                    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3) : "r"(src + o));
+                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + o), "r"(unpack_re4(w0)), "r"(unpack_re4(w1)),
+                                 "r"(unpack_re4(w2)), "r"(unpack_re4(w3))
+                                 : "memory");
+                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + Cfg::kPlaneBytes + o), "r"(unpack_im4(w0)),
+                                 "r"(unpack_im4(w1)), "r"(unpack_im4(w2)), "r"(unpack_im4(w3))
+                                 : "memory");
+                }
+                if (off) {
+#pragma unroll
+                    for (int q = 0; q < Cfg::kPlaneBytes / (128 * 16); ++q) {
+                        const uint32_t o = (uint32_t)(q * 128 + tid) * 16u;
+                        uint32_t w0, w1, w2, w3;
+                        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                     : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3)
+                                     : "r"(src + Cfg::kPlaneBytes + o));
+                        const uint32_t i0 = unpack_im4(w0), i1 = unpack_im4(w1), i2 = unpack_im4(w2), i3 = unpack_im4(w3);
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 2 * Cfg::kPlaneBytes + o), "r"(unpack_re4(w0)),
+                                     "r"(unpack_re4(w1)), "r"(unpack_re4(w2)), "r"(unpack_re4(w3))
+                                     : "memory");
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 3 * Cfg::kPlaneBytes + o), "r"(i0), "r"(i1), "r"(i2),
+                                     "r"(i3)
+                                     : "memory");
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 4 * Cfg::kPlaneBytes + o), "r"(negate4(i0)),
+                                     "r"(negate4(i1)), "r"(negate4(i2)), "r"(negate4(i3))
+                                     : "memory");
+                    }
+                }
+                ptx::fence_proxy_async_smem();       // my plane writes -> visible to the tensor core's smem reads
+                __syncwarp();
+                if (lane == 0) {
+                    ptx::mbar_arrive_local(bar_pk_empty(pslot));                       // packed slot may be refilled
+                    ptx::mbar_arrive_cluster(pl_full_leader + 8u * lslot);             // tell the leader's MMA thread
+                }
+            }
+        }
+    } else if (warp >= kWarpEpi0) {
+        // ===================================================== a4: epilogue warps
+        const uint32_t quarter = warp & 3u;                      // TMEM lanes [32*quarter, 32*quarter+32)
+        const uint32_t acc_empty_leader = ptx::mapa(bar_acc_empty, 0);
+        uint32_t unit = 0;
+        for (int sg = seg_begin; sg < seg_end; ++sg, ++unit) {
+            const Segment seg = p.segments[sg];
+            ptx::mbar_wait_cluster(bar_acc_full, unit & 1u);
+            ptx::tc_fence_after_sync();
+            const int row0 = (int)(rank * kBlock + quarter * 32);             // first row of this warp inside the super-block
+            const int rows_valid = p.n_inputs - seg.I * kSuper - row0;         // rows of this warp that are real inputs
+            const int cols_valid = min(kSuper, p.n_inputs - seg.J * kSuper);   // columns that are real inputs
+            int32_t *acc_cta = p.acc + ((size_t)seg.tile * 2 + rank) * (size_t)kAccElemsPerCta + quarter * 32 + lane;
+            if (rows_valid > 0) {
+                // R columns: on a diagonal super-tile only j >= i is ever read -> start at this warp's first row
+                const int r_begin = (seg.I == seg.J) ? row0 : 0;
+                for (int c = r_begin; c < cols_valid; c += 32) {
+                    uint32_t v[32];
+                    ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + (uint32_t)c, v);
+                    ptx::tmem_wait_ld();
+#pragma unroll
+                    for (int k = 0; k < 32; ++k) ptx::red_add_s32(acc_cta + (size_t)(c + k) * kBlock, (int32_t)v[k]);
+                }
+                for (int c = 0; c < cols_valid; c += 32) {
+                    uint32_t v[32];
+                    ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + 256u + (uint32_t)c, v);
+                    ptx::tmem_wait_ld();
+#pragma unroll
+                    for (int k = 0; k < 32; ++k) ptx::red_add_s32(acc_cta + (size_t)(256 + c + k) * kBlock, (int32_t)v[k]);
+                }
+            }
+            ptx::tc_fence_before_sync();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive_cluster(acc_empty_leader);          // TMEM may be overwritten by the next unit
+        }
+    }
+
+    // ---- teardown: everyone in both CTAs done with TMEM / peer smem before dealloc and exit ----
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::cluster_sync();
+    if (warp == kWarpTmem) {
+        ptx::tc_fence_after_sync();
+        ptx::tmem_dealloc<2>(tmem_base, kAccCols);
+    }
+}
+
+}  // namespace xc
