@@ -1,0 +1,292 @@
+#!/usr/bin/env python
+"""bench.py -- X-engine throughput on synthetic CHIME-shaped frames (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2|C4|C5|C3] [--impl reference]
+
+A "step" is one pass of the whole hot path over one frame: xcorr_process (TMA stage -> nibble unpack -> tcgen05
+int8 MMAs -> epilogue, rows a1..a4) followed by xcorr_read (the packed-triangle epilogue that ends the integration;
+BASELINE.json:configs[1] "one integration per frame").  `value` is input Gb/s with the frames already resident in
+HBM; `e2e` is the same metric through the streamed C-ABI path (row a5) with page-locked HOST frames and a HOST
+result, copies inside the timed region.  Inputs are synthetic (workloads.py) and larger than L2 (256 MiB frames,
+two of them alternating), so no flush is needed between iterations.
+
+Multi-GPU: the path does not shard ("replicas only"): --gpus N (under torchrun) runs N independent
+replicas, one per GPU, no collective on the data path; value = N frames' bits / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+import numpy as np  # noqa: E402
+
+import workloads as wl  # noqa: E402
+
+NOMINAL_INT8_TOPS = 4500.0  # dense int8, B200 nominal (2x the 2.25 PFLOP/s dense bf16 figure)
+# dram__bytes_read.sum + dram__bytes_write.sum of xengine_kernel<false> for one C2 launch, from the committed
+# ncu --set full capture summarised in profiles/ (None until a capture exists)
+NCU_TRAFFIC_BYTES = {"C2": None}
+
+
+def load_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_burst": d["bf16_tflops"], "bf16_sustained": d.get("bf16_tflops_sustained"),
+                "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.rows.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            c = [x.strip() for x in r.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg: wl.Config, seconds_hint: float = 12.0):
+    """Time the oracle, as it stands, on a bounded sample of `cfg`: a few whole channels of one frame."""
+    import oracle
+    oracle.build()
+    cores = oracle.threads()
+    n_ch = max(1, min(cfg.n_freq, 2 * cores if cfg.n_inputs <= 256 else 1))
+    t_samp = cfg.n_time if cfg.n_inputs <= 512 else min(cfg.n_time, 2048)
+    fr = wl.make_frame(cfg.kind, cfg.n_inputs, n_ch, t_samp, cfg.seed)
+    t0 = time.perf_counter()
+    oracle.planar(fr)
+    dt = time.perf_counter() - t0
+    bits = 8.0 * fr.nbytes
+    cmacs = n_ch * t_samp * cfg.n_pairs
+    return {"value": bits / dt / 1e9, "unit": "Gb/s", "cores": cores, "kind": "oracle",
+            "sample": f"oracle.planar (plain C, int64 accumulators, OpenMP) on {n_ch} of {cfg.n_freq} channels x "
+                      f"{t_samp} of {cfg.n_time} samples of one {cfg.name} frame (N={cfg.n_inputs}); {dt:.2f} s",
+            "cmac_per_s": cmacs / dt, "seconds": dt}
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle timed on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps, warm = max(1, min(args.steps, 5)), max(0, min(args.warmup, 1))
+    for _ in range(warm):
+        oracle_sample(cfg)
+    samples = [oracle_sample(cfg) for _ in range(steps)]
+    best = samples[-1]
+    v = statistics.mean(s["value"] for s in samples)
+    ms = statistics.mean(s["seconds"] for s in samples) * 1e3
+    line = {
+        "impl": "reference", "metric": "xengine_input_gbps", "value": v, "unit": "Gb/s", "n_gpus": args.gpus, "steps": steps,
+        "warmup": warm, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
+        "data": "synthetic", "config": {"workload": cfg.name, "n_inputs": cfg.n_inputs, "n_freq": cfg.n_freq,
+                                        "t_per_frame": cfg.n_time, "note": "each step = a bounded sample, see cpu_baseline.sample"},
+        "cpu_baseline": {"value": v, "unit": "Gb/s", "cores": best["cores"], "kind": "oracle", "sample": best["sample"]},
+        "e2e": {"value": v, "unit": "Gb/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "cmac_per_s": statistics.mean(s["cmac_per_s"] for s in samples), "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    cfg = wl.CONFIGS[args.config]
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+
+    import torch
+    import paper_1503_06189_b200 as xb
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    warm = max(3, args.warmup)
+    steps = max(1, args.steps)
+    peaks = load_peaks()
+
+    # ---- synthetic inputs, resident in HBM before the timed region: two distinct frames, alternating
+    n_distinct = 2
+    host_frames = [cfg.frame(k) for k in range(n_distinct)]
+    dev_frames = [torch.from_numpy(f).cuda() for f in host_frames]
+    x = xb.XCorr(cfg.n_inputs, cfg.n_freq, cfg.n_time)
+    out_dev = torch.empty((cfg.n_freq, cfg.n_pairs, 2), dtype=torch.int32, device="cuda")
+    st = torch.cuda.Stream()
+
+    def step(k):
+        x.process(dev_frames[k % n_distinct], st)
+        x.read(out_dev, st)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for k in range(warm):
+        step(k)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.15)
+    # -- timed region 1: K whole steps, CUDA events on the launching stream
+    launches0 = x.kernel_launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(st)
+    for k in range(steps):
+        step(k)
+    e1.record(st)
+    barrier()
+    total_ms = e0.elapsed_time(e1)
+    launches = x.kernel_launches - launches0
+    # -- timed region 2 (same loop, per-kernel events): duration of the dominant kernel (xengine_kernel = xcorr_process)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for k in range(steps):
+        evs[k][0].record(st)
+        x.process(dev_frames[k % n_distinct], st)
+        evs[k][1].record(st)
+        x.read(out_dev, st)
+    barrier()
+    kern_ms = [a.elapsed_time(b) for a, b in evs]
+    clocks = sampler.stop()
+
+    if dist is not None:
+        tt = torch.tensor([total_ms], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / steps
+    bits_per_frame = 8.0 * cfg.frame_bytes
+    value = world * bits_per_frame / (ms_per_step * 1e-3) / 1e9
+    cmac_per_s = world * cfg.cmacs_per_frame / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (tensor-bound: a dense int8 contraction)
+    k_ms = statistics.mean(kern_ms)
+    alg_ops = 8.0 * cfg.cmacs_per_frame              # 4 real MACs = 8 int8 ops per complex MAC, useful pairs i<=j only
+    achieved = alg_ops / (k_ms * 1e-3) / 1e12
+    peak = 2.0 * peaks["bf16_burst"]                 # int8 = 2 x bf16 (nominal ratio) x measured bf16 burst
+    roofline = {
+        "bound": "tensor", "kernel": "xengine_kernel (xcorr_process)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+        "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+        "peak_source": f"2 x bf16_tflops (burst) of MEASURED_PEAKS.json [{peaks['source']}]; int8:bf16 nominal ratio 4.5:2.25",
+        "kernel_ms": k_ms, "kernel_ms_min": min(kern_ms), "algorithmic_ops_per_launch": alg_ops,
+        "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
+        "hbm_gbs_staging": cfg.frame_bytes / (k_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"],
+    }
+
+    # ---- e2e: streamed C-ABI path, HOST frames in, HOST visibilities out, every step
+    e2e = None
+    if not args.no_e2e:
+        pinned = [torch.from_numpy(f).pin_memory() for f in host_frames]
+        out_host = torch.empty((cfg.n_freq, cfg.n_pairs, 2), dtype=torch.int32).pin_memory()
+        s = xb.XCorrStream(x, depth=2)
+        for k in range(2):
+            s.submit(pinned[k % n_distinct]); s.read(out_host)
+        barrier()
+        n_e2e = max(2, min(steps, 10))
+        t0 = time.perf_counter()
+        for k in range(n_e2e):
+            s.submit(pinned[k % n_distinct])
+            s.read(out_host)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            tt = torch.tensor([dt], device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt.item())
+        e2e = {"value": world * bits_per_frame * n_e2e / dt / 1e9, "unit": "Gb/s", "h2d_bytes_per_step": cfg.frame_bytes,
+               "d2h_bytes_per_step": cfg.output_bytes, "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3,
+               "api": "xcorr_stream_submit(pinned host frame) + xcorr_stream_read(pinned host out)"}
+        s.close()
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = oracle_sample(cfg)
+        cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "cmac_per_s")}
+
+    if rank == 0:
+        line = {
+            "metric": "xengine_input_gbps", "value": value, "unit": "Gb/s", "n_gpus": world, "steps": steps, "warmup": warm,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8",
+            "data": "synthetic",
+            "config": {"workload": cfg.name, "n_inputs": cfg.n_inputs, "n_freq": cfg.n_freq, "t_per_frame": cfg.n_time,
+                       "frame_bytes": cfg.frame_bytes, "step": "xcorr_process + xcorr_read (one integration per frame)",
+                       "l2": f"inputs larger than L2: {n_distinct} distinct {cfg.frame_bytes >> 20} MiB frames alternate",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU", "note": cfg.note},
+            "cmac_per_s": cmac_per_s,
+            "pct_int8_peak_nominal": 100.0 * 8.0 * cmac_per_s / world / (NOMINAL_INT8_TOPS * 1e12),
+            "pct_int8_peak_measured": 100.0 * 8.0 * cmac_per_s / world / (peak * 1e12),
+            "paper_context": "51.2 Gb/s per 3-GPU server, 819.2 Gb/s over 16 servers (PAPER.md Table I; other hardware)",
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        }
+        print(json.dumps(line), flush=True)
+    x.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,279 @@
+"""Python binding of libxcorr.so -- argument marshalling only; every step of the path runs in the CUDA kernels.
+
+The functions mirror include/xcorr.h one to one (same names, raw pointers as ints).  ``XCorr`` and
+``XCorrStream`` are thin conveniences that accept torch tensors (PyTorch is used for device / pinned memory and
+stream handles only).  There is no fallback: if the shared library is missing and cannot be built, or the device
+is not an sm_100 GPU, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+from . import _build
+
+__all__ = [
+    "XCORR_OK", "XCORR_EINVAL", "XCORR_EARCH", "XCORR_ENOMEM", "XCORR_ECUDA", "XCORR_EOVERFLOW",
+    "XCorrError", "lib", "xcorr_create", "xcorr_process", "xcorr_read", "xcorr_destroy", "xcorr_strerror",
+    "xcorr_last_cuda_error", "xcorr_frame_bytes", "xcorr_output_bytes", "xcorr_kernel_launches",
+    "xcorr_stream_create", "xcorr_stream_submit", "xcorr_stream_sync", "xcorr_stream_read", "xcorr_stream_destroy",
+    "xcorr_debug_schedule", "xcorr_debug_stage_samples", "xcorr_debug_process_simt", "XCorr", "XCorrStream",
+]
+
+XCORR_OK, XCORR_EINVAL, XCORR_EARCH, XCORR_ENOMEM, XCORR_ECUDA, XCORR_EOVERFLOW = 0, -1, -2, -3, -4, -5
+
+_lib = None
+
+
+class XCorrError(RuntimeError):
+    def __init__(self, code: int, what: str, cuda_error: int = 0):
+        self.code = code
+        self.cuda_error = cuda_error
+        msg = f"{what}: {xcorr_strerror(code)} (code {code})"
+        if cuda_error:
+            msg += f" [cudaError {cuda_error}]"
+        super().__init__(msg)
+
+
+def lib() -> ctypes.CDLL:
+    """Load (building first if the sources are newer) libxcorr.so.  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path: Path = _build.LIB
+    if _build.needs_build():
+        try:
+            _build.build()
+        except Exception as e:  # no nvcc on this box
+            if not path.exists():
+                raise RuntimeError(f"libxcorr.so is missing and could not be built: {e}") from e
+    L = ctypes.CDLL(str(path))
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    L.xcorr_create.argtypes = [ci, ci, ci, ctypes.POINTER(vp)]
+    L.xcorr_create.restype = ci
+    L.xcorr_process.argtypes = [vp, vp, vp]
+    L.xcorr_process.restype = ci
+    L.xcorr_read.argtypes = [vp, vp, vp]
+    L.xcorr_read.restype = ci
+    L.xcorr_destroy.argtypes = [vp]
+    L.xcorr_destroy.restype = None
+    L.xcorr_strerror.argtypes = [ci]
+    L.xcorr_strerror.restype = ctypes.c_char_p
+    L.xcorr_last_cuda_error.argtypes = [vp]
+    L.xcorr_last_cuda_error.restype = ci
+    L.xcorr_frame_bytes.argtypes = [vp]
+    L.xcorr_frame_bytes.restype = ctypes.c_size_t
+    L.xcorr_output_bytes.argtypes = [vp]
+    L.xcorr_output_bytes.restype = ctypes.c_size_t
+    L.xcorr_kernel_launches.argtypes = [vp]
+    L.xcorr_kernel_launches.restype = ctypes.c_uint64
+    L.xcorr_stream_create.argtypes = [vp, ci, ctypes.POINTER(vp)]
+    L.xcorr_stream_create.restype = ci
+    L.xcorr_stream_submit.argtypes = [vp, vp]
+    L.xcorr_stream_submit.restype = ci
+    L.xcorr_stream_sync.argtypes = [vp]
+    L.xcorr_stream_sync.restype = ci
+    L.xcorr_stream_read.argtypes = [vp, vp]
+    L.xcorr_stream_read.restype = ci
+    L.xcorr_stream_destroy.argtypes = [vp]
+    L.xcorr_stream_destroy.restype = None
+    L.xcorr_debug_schedule.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ctypes.c_int32), ci, ctypes.POINTER(ctypes.c_int32)]
+    L.xcorr_debug_schedule.restype = ci
+    L.xcorr_debug_stage_samples.argtypes = []
+    L.xcorr_debug_stage_samples.restype = ci
+    L.xcorr_debug_process_simt.argtypes = [vp, vp, vp]
+    L.xcorr_debug_process_simt.restype = ci
+    _lib = L
+    return L
+
+
+# ------------------------------------------------------------------------------------------ raw C-ABI mirrors
+def xcorr_strerror(code: int) -> str:
+    return lib().xcorr_strerror(int(code)).decode()
+
+
+def xcorr_create(n_inputs: int, n_freq: int, t_per_frame: int) -> tuple[int, int]:
+    """-> (code, handle).  handle is 0 on failure."""
+    h = ctypes.c_void_p()
+    rc = lib().xcorr_create(int(n_inputs), int(n_freq), int(t_per_frame), ctypes.byref(h))
+    return rc, (h.value or 0)
+
+
+def xcorr_process(handle: int, packed_frame_dev: int, cuda_stream: int = 0) -> int:
+    return lib().xcorr_process(handle, packed_frame_dev, cuda_stream)
+
+
+def xcorr_read(handle: int, upper_triangle_out: int, cuda_stream: int = 0) -> int:
+    return lib().xcorr_read(handle, upper_triangle_out, cuda_stream)
+
+
+def xcorr_destroy(handle: int) -> None:
+    lib().xcorr_destroy(handle)
+
+
+def xcorr_last_cuda_error(handle: int) -> int:
+    return lib().xcorr_last_cuda_error(handle)
+
+
+def xcorr_frame_bytes(handle: int) -> int:
+    return lib().xcorr_frame_bytes(handle)
+
+
+def xcorr_output_bytes(handle: int) -> int:
+    return lib().xcorr_output_bytes(handle)
+
+
+def xcorr_kernel_launches(handle: int) -> int:
+    return lib().xcorr_kernel_launches(handle)
+
+
+def xcorr_stream_create(handle: int, depth: int = 2) -> tuple[int, int]:
+    s = ctypes.c_void_p()
+    rc = lib().xcorr_stream_create(handle, int(depth), ctypes.byref(s))
+    return rc, (s.value or 0)
+
+
+def xcorr_stream_submit(stream: int, frame_host: int) -> int:
+    return lib().xcorr_stream_submit(stream, frame_host)
+
+
+def xcorr_stream_sync(stream: int) -> int:
+    return lib().xcorr_stream_sync(stream)
+
+
+def xcorr_stream_read(stream: int, upper_triangle_out: int) -> int:
+    return lib().xcorr_stream_read(stream, upper_triangle_out)
+
+
+def xcorr_stream_destroy(stream: int) -> None:
+    lib().xcorr_stream_destroy(stream)
+
+
+def xcorr_debug_stage_samples() -> int:
+    return lib().xcorr_debug_stage_samples()
+
+
+def xcorr_debug_schedule(n_inputs: int, n_freq: int, t_per_frame: int, n_workers: int):
+    """-> (segments int32[K][6] = f, I, J, stage_begin, stage_end, tile ; worker_begin int32[n_workers+1]).  No GPU needed."""
+    import numpy as np
+    n = lib().xcorr_debug_schedule(n_inputs, n_freq, t_per_frame, n_workers, None, 0, None)
+    if n < 0:
+        raise XCorrError(n, "xcorr_debug_schedule")
+    seg = np.zeros((max(n, 1), 6), dtype=np.int32)
+    wb = np.zeros(n_workers + 1, dtype=np.int32)
+    n2 = lib().xcorr_debug_schedule(n_inputs, n_freq, t_per_frame, n_workers,
+                                    seg.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), n,
+                                    wb.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)))
+    assert n2 == n
+    return seg[:n], wb
+
+
+def xcorr_debug_process_simt(handle: int, packed_frame_dev: int, cuda_stream: int = 0) -> int:
+    return lib().xcorr_debug_process_simt(handle, packed_frame_dev, cuda_stream)
+
+
+# ------------------------------------------------------------------------------------------ torch conveniences
+def _stream_handle(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+class XCorr:
+    """One (N, F, T) correlator handle.  ``process`` accumulates a device frame, ``read`` ends the integration."""
+
+    def __init__(self, n_inputs: int, n_freq: int, t_per_frame: int):
+        rc, h = xcorr_create(n_inputs, n_freq, t_per_frame)
+        if rc != XCORR_OK:
+            raise XCorrError(rc, "xcorr_create")
+        self.handle = h
+        self.n_inputs, self.n_freq, self.t_per_frame = n_inputs, n_freq, t_per_frame
+        self.n_pairs = n_inputs * (n_inputs + 1) // 2
+
+    @property
+    def frame_bytes(self) -> int:
+        return xcorr_frame_bytes(self.handle)
+
+    @property
+    def output_bytes(self) -> int:
+        return xcorr_output_bytes(self.handle)
+
+    @property
+    def kernel_launches(self) -> int:
+        return xcorr_kernel_launches(self.handle)
+
+    def _check(self, rc: int, what: str):
+        if rc != XCORR_OK:
+            raise XCorrError(rc, what, xcorr_last_cuda_error(self.handle))
+
+    def process(self, frame_dev, stream=None) -> None:
+        """frame_dev: torch uint8 CUDA tensor of N*F*T bytes ([T][F][N]), contiguous."""
+        if not frame_dev.is_cuda or not frame_dev.is_contiguous() or frame_dev.numel() * frame_dev.element_size() != self.frame_bytes:
+            raise ValueError("frame_dev must be a contiguous CUDA tensor of exactly frame_bytes bytes")
+        self._check(xcorr_process(self.handle, frame_dev.data_ptr(), _stream_handle(stream)), "xcorr_process")
+
+    def process_simt_debug(self, frame_dev, stream=None) -> None:
+        self._check(xcorr_debug_process_simt(self.handle, frame_dev.data_ptr(), _stream_handle(stream)), "xcorr_debug_process_simt")
+
+    def read(self, out=None, stream=None):
+        """Write int32[F][P][2] into ``out`` (CUDA or CPU torch int32 tensor; allocated on the device if None)."""
+        import torch
+        if out is None:
+            out = torch.empty((self.n_freq, self.n_pairs, 2), dtype=torch.int32, device="cuda")
+        if out.dtype != torch.int32 or not out.is_contiguous() or out.numel() * 4 != self.output_bytes:
+            raise ValueError("out must be a contiguous int32 tensor of output_bytes bytes")
+        self._check(xcorr_read(self.handle, out.data_ptr(), _stream_handle(stream)), "xcorr_read")
+        return out
+
+    def close(self) -> None:
+        if getattr(self, "handle", 0):
+            xcorr_destroy(self.handle)
+            self.handle = 0
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class XCorrStream:
+    """Double-buffered pinned-host -> device frame stream over an ``XCorr`` (hot-path row a5)."""
+
+    def __init__(self, xc: XCorr, depth: int = 2):
+        rc, s = xcorr_stream_create(xc.handle, depth)
+        if rc != XCORR_OK:
+            raise XCorrError(rc, "xcorr_stream_create", xcorr_last_cuda_error(xc.handle))
+        self.xc, self.stream = xc, s
+
+    def submit(self, frame_host) -> None:
+        """frame_host: contiguous CPU uint8 tensor (pinned for overlap) or numpy array of frame_bytes bytes."""
+        if hasattr(frame_host, "data_ptr"):
+            ptr, nbytes = frame_host.data_ptr(), frame_host.numel() * frame_host.element_size()
+        else:
+            ptr, nbytes = frame_host.ctypes.data, frame_host.nbytes
+        if nbytes != self.xc.frame_bytes:
+            raise ValueError("frame_host must hold exactly frame_bytes bytes")
+        self.xc._check(xcorr_stream_submit(self.stream, ptr), "xcorr_stream_submit")
+
+    def sync(self) -> None:
+        self.xc._check(xcorr_stream_sync(self.stream), "xcorr_stream_sync")
+
+    def read(self, out):
+        ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        self.xc._check(xcorr_stream_read(self.stream, ptr), "xcorr_stream_read")
+        return out
+
+    def close(self) -> None:
+        if getattr(self, "stream", 0):
+            xcorr_stream_destroy(self.stream)
+            self.stream = 0
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

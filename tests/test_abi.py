@@ -1,0 +1,77 @@
+"""The C-ABI library loads and exports every symbol include/*.h declares (no compute calls: CPU only)."""
+import ctypes
+import re
+from pathlib import Path
+
+import pytest
+
+import paper_1503_06189_b200 as xb
+
+INCLUDE = Path(__file__).resolve().parent.parent / "include"
+
+
+def _declared_symbols():
+    names = []
+    for h in sorted(INCLUDE.glob("*.h")):
+        text = re.sub(r"/\*.*?\*/", "", h.read_text(), flags=re.S)
+        for m in re.finditer(r"\b(xcorr_[a-z0-9_]+)\s*\(", text):
+            names.append(m.group(1))
+    return sorted(set(names))
+
+
+def test_headers_declare_the_three_calls():
+    names = _declared_symbols()
+    for must in ("xcorr_create", "xcorr_process", "xcorr_read", "xcorr_destroy", "xcorr_strerror",
+                 "xcorr_stream_create", "xcorr_stream_submit", "xcorr_stream_read"):
+        assert must in names
+
+
+@pytest.mark.parametrize("name", _declared_symbols())
+def test_symbol_exported(name):
+    L = xb.lib()
+    assert getattr(L, name) is not None
+
+
+def test_no_torch_types_in_abi():
+    for h in INCLUDE.glob("*.h"):
+        code = re.sub(r"/\*.*?\*/", "", h.read_text(), flags=re.S)   # comments may mention torch pin_memory
+        assert "torch" not in code.lower() and "at::" not in code and "#include <cuda" not in code
+
+
+def test_strerror_is_total():
+    for code in range(-8, 2):
+        s = xb.xcorr_strerror(code)
+        assert isinstance(s, str) and s
+    assert xb.xcorr_strerror(xb.XCORR_OK) == "ok"
+    assert "overflow" in xb.xcorr_strerror(xb.XCORR_EOVERFLOW)
+
+
+@pytest.mark.parametrize("shape", [(0, 4, 16), (16, 0, 16), (16, 4, 0), (-16, 4, 16), (24, 4, 16), (8, 1, 1), (250, 2, 64)])
+def test_create_rejects_bad_shapes_without_touching_the_gpu(shape):
+    rc, h = xb.xcorr_create(*shape)
+    assert rc == xb.XCORR_EINVAL and h == 0
+
+
+def test_null_handles_are_harmless():
+    assert xb.xcorr_frame_bytes(0) == 0
+    assert xb.xcorr_output_bytes(0) == 0
+    assert xb.xcorr_kernel_launches(0) == 0
+    assert xb.xcorr_last_cuda_error(0) == 0
+    xb.xcorr_destroy(0)
+    xb.xcorr_stream_destroy(0)
+    assert xb.xcorr_process(0, 0, 0) == xb.XCORR_EINVAL
+    assert xb.xcorr_read(0, 0, 0) == xb.XCORR_EINVAL
+    assert xb.xcorr_stream_submit(0, 0) == xb.XCORR_EINVAL
+
+
+def test_create_fails_loudly_without_a_gpu():
+    try:
+        import torch
+        if torch.cuda.is_available():
+            pytest.skip("GPU present")
+    except ImportError:
+        pass
+    rc, h = xb.xcorr_create(16, 4, 256)
+    assert rc in (xb.XCORR_ECUDA, xb.XCORR_EARCH) and h == 0
+    with pytest.raises(xb.XCorrError):
+        xb.XCorr(16, 4, 256)
