@@ -39,10 +39,13 @@ __device__ __forceinline__ void mbar_arrive_local(uint32_t bar)
 {
     asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// arrive on a barrier given by a shared::cluster address (own or peer CTA), cluster-scope release
+// arrive on a barrier given by a shared::cluster address (own or peer CTA).  Default .release.cta semantics on
+// purpose: a cluster-scope release costs MEMBAR.ALL.GPU + ERRBAR per arrive (measured: 18 % of all stall samples,
+// profiles/r01_dev_notes.md); the data handed over lives in the arriving CTA's own smem and is published to the
+// tensor core by fence.proxy.async, the arrive itself is only the signal.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster_addr)
 {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
 {
@@ -62,14 +65,15 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         "}" ::"r"(bar), "r"(parity)
         : "memory");
 }
-// same, acquire at cluster scope (the completing arrivals came from the peer CTA / a multicast commit)
+// same wait for barriers completed by the peer CTA / a multicast tcgen05.commit.  Kept as a separate name for
+// readability; a cluster-scope acquire here makes ptxas emit CCTL.IVALL (L1 invalidate) after every wait.
 __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
 {
     asm volatile(
         "{\n\t"
         ".reg .pred p;\n\t"
         "LAB_WAIT:\n\t"
-        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
         "@p bra LAB_DONE;\n\t"
         "bra LAB_WAIT;\n\t"
         "LAB_DONE:\n\t"

@@ -37,8 +37,14 @@ struct KernelCfg {
     static constexpr int kPlanes = kOffDiag ? 5 : 2;               // h_a l_a [h_b l_b -l_b]
     static constexpr int kPackedStageBytes = kPackedBlocks * kPlaneBytes;
     static constexpr int kPlaneStageBytes = kPlanes * kPlaneBytes;
-    static constexpr int kPackedStages = kOffDiag ? 3 : 4;
-    static constexpr int kPlaneStages = kOffDiag ? 3 : 6;
+#ifndef XC_PACKED_STAGES_DIAG
+#define XC_PACKED_STAGES_DIAG 4
+#endif
+#ifndef XC_PLANE_STAGES_DIAG
+#define XC_PLANE_STAGES_DIAG 6
+#endif
+    static constexpr int kPackedStages = kOffDiag ? 3 : XC_PACKED_STAGES_DIAG;
+    static constexpr int kPlaneStages = kOffDiag ? 3 : XC_PLANE_STAGES_DIAG;
     static constexpr int kSmemData = kPackedStages * kPackedStageBytes + kPlaneStages * kPlaneStageBytes;
     static constexpr int kSmemBytes = kSmemData + 1024 /*align slack*/ + 1024 /*barriers*/;
 };
@@ -277,15 +283,19 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                     uint32_t v[32];
                     ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + (uint32_t)c, v);
                     ptx::tmem_wait_ld();
+#ifndef XC_DEBUG_SKIP_RED
 #pragma unroll
                     for (int k = 0; k < 32; ++k) ptx::red_add_s32(acc_cta + (size_t)(c + k) * kBlock, (int32_t)v[k]);
+#endif
                 }
                 for (int c = 0; c < cols_valid; c += 32) {
                     uint32_t v[32];
                     ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + 256u + (uint32_t)c, v);
                     ptx::tmem_wait_ld();
+#ifndef XC_DEBUG_SKIP_RED
 #pragma unroll
                     for (int k = 0; k < 32; ++k) ptx::red_add_s32(acc_cta + (size_t)(256 + c + k) * kBlock, (int32_t)v[k]);
+#endif
                 }
             }
             ptx::tc_fence_before_sync();
