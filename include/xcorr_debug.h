@@ -18,7 +18,7 @@ extern "C" {
  * tiles", BASELINE.json:north_star (b)); it is cut along time into stages of xcorr_debug_stage_samples()
  * samples and the stages are dealt to workers.
  * Returns the number of segments (>= 0) or XCORR_EINVAL.  With non-NULL outputs writes
- * segments_out[k][6] = {f, I, J, stage_begin, stage_end, tile} (capacity max_segments) and
+ * segments_out[k][7] = {f, I, J, stage_begin, stage_end, tile, slot} (capacity max_segments) and
  * worker_begin_out[n_workers + 1].
  */
 int xcorr_debug_schedule(int n_inputs, int n_freq, int t_per_frame, int n_workers,

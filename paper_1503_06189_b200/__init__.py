@@ -154,12 +154,12 @@ def xcorr_debug_stage_samples() -> int:
 
 
 def xcorr_debug_schedule(n_inputs: int, n_freq: int, t_per_frame: int, n_workers: int):
-    """-> (segments int32[K][6] = f, I, J, stage_begin, stage_end, tile ; worker_begin int32[n_workers+1]).  No GPU needed."""
+    """-> (segments int32[K][7] = f, I, J, stage_begin, stage_end, tile, slot ; worker_begin int32[n_workers+1]).  No GPU needed."""
     import numpy as np
     n = lib().xcorr_debug_schedule(n_inputs, n_freq, t_per_frame, n_workers, None, 0, None)
     if n < 0:
         raise XCorrError(n, "xcorr_debug_schedule")
-    seg = np.zeros((max(n, 1), 6), dtype=np.int32)
+    seg = np.zeros((max(n, 1), 7), dtype=np.int32)
     wb = np.zeros(n_workers + 1, dtype=np.int32)
     n2 = lib().xcorr_debug_schedule(n_inputs, n_freq, t_per_frame, n_workers,
                                     seg.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), n,

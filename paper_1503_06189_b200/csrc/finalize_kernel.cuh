@@ -1,9 +1,10 @@
-// finalize_kernel.cuh -- xcorr_read's kernel: device accumulator (layout.hpp) -> packed upper triangle
+// finalize_kernel.cuh -- xcorr_read's kernel: accumulator slots (layout.hpp) -> packed upper triangle
 // int32[F][P][2] (R4), and the SIMT cross-check kernel used only by the tests.
 //
-// The accumulator is column-major per CTA tile (row = TMEM lane is the fast index), the output is row-major
-// in (i, j); each block turns one 32 x 32 patch around through shared memory so that both sides are
-// 128-byte coalesced.  On diagonal super-tiles Im V[i,j] = X[i,j] - X[j,i] (layout.hpp).
+// A slot is [r][col/4][row][4] (row = TMEM lane fast), the output is row-major in (i, j).  Each block turns one
+// 32 x 32 patch around through shared memory so that both sides are coalesced: 16-byte vector reads along the row
+// index, 8-byte (re, im) writes along j.  The slots of a super-tile (one per work segment that summed part of
+// its time range) are added here.  On diagonal super-tiles Im V[i,j] = X[i,j] - X[j,i] (layout.hpp).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -12,49 +13,61 @@
 
 namespace xc {
 
-__device__ __forceinline__ const int32_t *acc_elem(const int32_t *acc, int nst, int nb, int f, int i, int j, int q_cols)
+// sum over the tile's slots of the 4 consecutive columns [col4*4, col4*4+4) of row `row`, CTA half r
+__device__ __forceinline__ int4 slot_sum_v4(const int32_t *__restrict__ acc, int slot_begin, int slot_end, int r, int col4, int row)
 {
-    // element for row input i, column input j (i's super-block <= j's); q_cols = 0 -> R, 256 -> Q
-    const int I = i / kSuper, J = j / kSuper;
-    const int tile = f * nst + supertile_index(nb, I, J);
-    const int r = (i % kSuper) / kBlock;
-    return acc + ((size_t)tile * 2 + r) * (size_t)kAccElemsPerCta + (size_t)(q_cols + j % kSuper) * kBlock + (i % kBlock);
+    int4 s = make_int4(0, 0, 0, 0);
+    for (int sl = slot_begin; sl < slot_end; ++sl) {
+        const int4 v = *reinterpret_cast<const int4 *>(acc + (size_t)sl * kAccElemsPerSlot + (size_t)r * kAccElemsPerCta +
+                                                       ((size_t)col4 * kBlock + row) * 4);
+        s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
+    }
+    return s;
 }
 
-// grid (nt, nt, F), nt = ceil(N / 32); block (32, 8)
-__global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict__ acc, int32_t *__restrict__ out, int n_inputs)
+// grid (nt, nt, F), nt = ceil(N / 32); block 256 threads
+__global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict__ acc, const int32_t *__restrict__ tile_slot_begin,
+                                                        int32_t *__restrict__ out, int n_inputs)
 {
     const int bj = blockIdx.x, bi = blockIdx.y, f = blockIdx.z;
     if (bj < bi) return;
-    __shared__ int32_t sR[32][33];
-    __shared__ int32_t sQ[32][33];
-    const int tx = threadIdx.x, ty = threadIdx.y;
+    __shared__ int32_t sR[32][33];   // [col][row]
+    __shared__ int32_t sQ[32][33];   // [col][row]
+    __shared__ int32_t sX[32][33];   // [row j][col i] of the transposed patch (diagonal super-tiles only)
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;   // ty in 0..7
     const int nb = n_super(n_inputs), nst = n_supertiles(nb);
     const int i0 = bi * 32, j0 = bj * 32;
-    const bool diag_super = (i0 / kSuper) == (j0 / kSuper);
+    const int I = i0 / kSuper, J = j0 / kSuper;
+    const bool diag_super = (I == J);
+    const int tile = f * nst + supertile_index(nb, I, J);
+    const int sb = tile_slot_begin[tile], se = tile_slot_begin[tile + 1];
 
-    // phase 1: coalesced reads along the row index (tx <-> row i0 + tx), one column per ty step
-    for (int cc = ty; cc < 32; cc += 8) {
-        const int i = i0 + tx, j = j0 + cc;
-        int32_t r = 0, q = 0;
-        if (i < n_inputs && j < n_inputs) {
-            r = *acc_elem(acc, nst, nb, f, i, j, 0);
-            q = *acc_elem(acc, nst, nb, f, i, j, 256);
+    // phase 1: thread (tx = row, ty = group of 4 columns): 16-byte loads, 512 B contiguous per warp
+    {
+        const int il = (i0 % kSuper) + tx;            // row inside the super-block
+        const int r = il / kBlock, row = il % kBlock;
+        const int c4 = ((j0 % kSuper) >> 2) + ty;     // column group inside the super-block
+        const int4 vr = slot_sum_v4(acc, sb, se, r, c4, row);
+        const int4 vq = slot_sum_v4(acc, sb, se, r, 64 + c4, row);
+        sR[4 * ty + 0][tx] = vr.x; sR[4 * ty + 1][tx] = vr.y; sR[4 * ty + 2][tx] = vr.z; sR[4 * ty + 3][tx] = vr.w;
+        sQ[4 * ty + 0][tx] = vq.x; sQ[4 * ty + 1][tx] = vq.y; sQ[4 * ty + 2][tx] = vq.z; sQ[4 * ty + 3][tx] = vq.w;
+        if (diag_super) {
+            // X[j][i] for rows j in [j0, j0+32), columns i in [i0, i0+32)
+            const int jl = (j0 % kSuper) + tx;
+            const int4 vx = slot_sum_v4(acc, sb, se, jl / kBlock, 64 + ((i0 % kSuper) >> 2) + ty, jl % kBlock);
+            sX[tx][4 * ty + 0] = vx.x; sX[tx][4 * ty + 1] = vx.y; sX[tx][4 * ty + 2] = vx.z; sX[tx][4 * ty + 3] = vx.w;
         }
-        sR[cc][tx] = r;
-        sQ[cc][tx] = q;
     }
     __syncthreads();
-    // phase 2: tx <-> column j0 + tx, one output row per ty step; X[j,i] is read coalesced along j
+    // phase 2: tx <-> column j0 + tx, one output row per ty step: 8-byte (re, im) writes, 256 B contiguous per warp
     const long long P = (long long)n_inputs * (n_inputs + 1) / 2;
     for (int ic = ty; ic < 32; ic += 8) {
         const int i = i0 + ic, j = j0 + tx;
-        if (i < n_inputs && j < n_inputs && i <= j) {
-            int32_t re = sR[tx][ic];
+        if (j < n_inputs && i <= j) {
+            const int32_t re = sR[tx][ic];
             int32_t im = sQ[tx][ic];
-            if (diag_super) im = (i == j) ? 0 : im - *acc_elem(acc, nst, nb, f, j, i, 256);
-            int2 v = make_int2(re, im);
-            *reinterpret_cast<int2 *>(out + ((long long)f * P + pair_index(n_inputs, i, j)) * 2) = v;
+            if (diag_super) im = (i == j) ? 0 : im - sX[tx][ic];
+            *reinterpret_cast<int2 *>(out + ((long long)f * P + pair_index(n_inputs, i, j)) * 2) = make_int2(re, im);
         }
     }
 }
@@ -62,9 +75,11 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
 // ------------------------------------------------------------------------------------------------
 // SIMT cross-check ("second opinion" for the GPU tests at sizes where the CPU oracle takes minutes).
 // One thread per accumulator element, plain integer loop over t.  NOT used by xcorr_process.
+// Adds into the FIRST slot of each tile (the caller zeroes all slots at the start of an integration).
 // grid: n_tiles * 2 * (128 / 8) blocks, block 256 threads (thread <-> column), 8 rows per block.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) simt_reference_kernel(const uint8_t *__restrict__ frame, int32_t *acc, int n_inputs, int n_freq,
+__global__ void __launch_bounds__(256) simt_reference_kernel(const uint8_t *__restrict__ frame, int32_t *acc,
+                                                             const int32_t *__restrict__ tile_slot_begin, int n_inputs, int n_freq,
                                                              int n_time)
 {
     constexpr int kRows = 8;
@@ -98,11 +113,11 @@ __global__ void __launch_bounds__(256) simt_reference_kernel(const uint8_t *__re
             accQ[k] += diag ? li * hj : li * hj - hi * lj;
         }
     }
-    int32_t *base = acc + ((size_t)tile * 2 + r) * (size_t)kAccElemsPerCta;
+    int32_t *base = acc + (size_t)tile_slot_begin[tile] * kAccElemsPerSlot;
 #pragma unroll
     for (int k = 0; k < kRows; ++k) {
-        atomicAdd(base + (size_t)col * kBlock + row_base + k, accR[k]);
-        atomicAdd(base + (size_t)(256 + col) * kBlock + row_base + k, accQ[k]);
+        atomicAdd(base + slot_offset(r, col, row_base + k), accR[k]);
+        atomicAdd(base + slot_offset(r, 256 + col, row_base + k), accQ[k]);
     }
 }
 

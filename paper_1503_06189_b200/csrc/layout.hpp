@@ -4,10 +4,13 @@
 // tcgen05 MMA, M = 256 = two CTAs x 128 TMEM lanes, N = 256).  Only super-tiles (I <= J) on or above
 // the diagonal exist ("computes only upper-triangle tiles", BASELINE.json:north_star (b)).
 //
-// Device accumulator ("kernels add to the output of the last run") -- TMEM-native order so
-// that the epilogue's adds are 128-byte coalesced with no transposition:
+// Device accumulator ("kernels add to the output of the last run").  A super-tile may be summed
+// over time by several work segments (schedule.hpp); every segment owns one SLOT, so the epilogue needs no
+// atomics: it stores (first frame of an integration) or load-add-stores (later frames) its own slot, and
+// xcorr_read adds the slots of a tile together.  Slot layout -- TMEM-native, so that one warp's 16-byte
+// vector accesses are 512-byte contiguous:
 //
-//   acc[f][st(I,J)][r][col][row]   int32,   r in {0,1}, col in [0,512), row in [0,128)
+//   acc[slot][r][col / 4][row][col % 4]   int32,   r in {0,1}, col in [0,512), row in [0,128)
 //
 //     row          = TMEM lane       : input  i = 256*I + 128*r + row
 //     col in [0,256)  "R" columns    : input  j = 256*J + col          value  Re V[i,j] = sum h_i h_j + l_i l_j
@@ -15,7 +18,8 @@
 //         I <  J :  value  Im V[i,j] = sum l_i h_j - h_i l_j
 //         I == J :  value  X[i,j]    = sum l_i h_j ;   Im V[i,j] = X[i,j] - X[j,i]  is formed by xcorr_read
 //
-// Lower-triangle R entries of diagonal super-tiles and anything with i >= N or j >= N are never read.
+// Lower-triangle R entries of diagonal super-tiles and anything with i >= N or j >= N are never read
+// (and mostly never written).
 #pragma once
 #include <cstdint>
 
@@ -25,7 +29,7 @@ constexpr int kBlock = 128;        // inputs per CTA row block (TMEM lanes)
 constexpr int kSuper = 256;        // inputs per super-block (CTA pair)
 constexpr int kAccCols = 512;      // TMEM columns per CTA: 256 R + 256 Q
 constexpr int kAccElemsPerCta = kAccCols * kBlock;          // 65536 int32
-constexpr int kAccElemsPerTile = 2 * kAccElemsPerCta;        // 131072 int32 = 512 KiB
+constexpr int kAccElemsPerSlot = 2 * kAccElemsPerCta;        // 131072 int32 = 512 KiB
 
 __host__ __device__ inline int n_super(int n_inputs) { return (n_inputs + kSuper - 1) / kSuper; }
 __host__ __device__ inline int n_supertiles(int nb) { return nb * (nb + 1) / 2; }
@@ -33,5 +37,10 @@ __host__ __device__ inline int n_supertiles(int nb) { return nb * (nb + 1) / 2; 
 __host__ __device__ inline int supertile_index(int nb, int I, int J) { return I * (2 * nb - I + 1) / 2 + (J - I); }
 // R4: packed output pair index
 __host__ __device__ inline long long pair_index(long long n, long long i, long long j) { return i * (2 * n - i + 1) / 2 + (j - i); }
+// int32 offset of (r, col, row) inside a slot
+__host__ __device__ inline size_t slot_offset(int r, int col, int row)
+{
+    return (size_t)r * kAccElemsPerCta + ((size_t)(col >> 2) * kBlock + row) * 4 + (col & 3);
+}
 
 }  // namespace xc

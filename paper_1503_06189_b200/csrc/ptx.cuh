@@ -172,10 +172,16 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&v)[32])
 }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-// ---------------------------------------------------------------- global reductions
-__device__ __forceinline__ void red_add_s32(int32_t *addr, int32_t v)
+// ---------------------------------------------------------------- global 16-byte accesses (accumulator slots)
+__device__ __forceinline__ void st_global_v4(int32_t *addr, int32_t a, int32_t b, int32_t c, int32_t d)
 {
-    asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(addr), "r"(v) : "memory");
+    asm volatile("st.global.v4.s32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ int4 ld_global_v4(const int32_t *addr)
+{
+    int4 r;
+    asm volatile("ld.global.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(addr) : "memory");
+    return r;
 }
 
 // ---------------------------------------------------------------- descriptors

@@ -13,6 +13,7 @@
 //   * the stages of the remaining items are dealt out as contiguous runs so that every worker ends
 //     with (nearly) the same total cost ("water filling").
 // Every (item, stage) is assigned to exactly one worker (checked by tests/test_host_logic.py).
+// Each segment owns one accumulator SLOT (layout.hpp); a tile's slots are numbered contiguously.
 #pragma once
 #include <algorithm>
 #include <cstdint>
@@ -27,8 +28,9 @@ struct Segment {          // 32 bytes, read by the kernel
     int32_t I, J;         // super-block row / column (I <= J)
     int32_t stage_begin;  // [stage_begin, stage_end) in units of kStageT samples
     int32_t stage_end;
-    int32_t tile;         // f * n_supertiles + supertile_index(I, J)  (accumulator tile)
-    int32_t pad0, pad1;
+    int32_t tile;         // f * n_supertiles + supertile_index(I, J)
+    int32_t slot;         // accumulator slot owned by this segment (layout.hpp)
+    int32_t pad1;
 };
 
 struct Schedule {
@@ -36,6 +38,7 @@ struct Schedule {
     int n_stages = 0;                 // stages per item = ceil(T / kStageT)
     std::vector<Segment> segments;    // grouped by worker
     std::vector<int32_t> worker_begin;  // size n_workers + 1, offsets into segments
+    std::vector<int32_t> tile_slot_begin;  // size n_tiles + 1: slots [b[t], b[t+1]) belong to tile t
 };
 
 inline Schedule make_schedule(int n_inputs, int n_freq, int n_time, int n_workers)
@@ -107,6 +110,19 @@ inline Schedule make_schedule(int n_inputs, int n_freq, int n_time, int n_worker
                 st += take;
             }
         }
+    }
+
+    // slots: one per segment, numbered in (tile, stage_begin) order so that a tile's slots are contiguous
+    {
+        std::vector<Segment *> all;
+        for (auto &v : per) for (auto &g : v) all.push_back(&g);
+        std::sort(all.begin(), all.end(), [](const Segment *a, const Segment *b) {
+            return a->tile != b->tile ? a->tile < b->tile : a->stage_begin < b->stage_begin;
+        });
+        const int n_tiles = n_freq * nst;
+        s.tile_slot_begin.assign(n_tiles + 1, 0);
+        for (size_t k = 0; k < all.size(); ++k) { all[k]->slot = (int32_t)k; s.tile_slot_begin[all[k]->tile + 1] += 1; }
+        for (int t = 0; t < n_tiles; ++t) s.tile_slot_begin[t + 1] += s.tile_slot_begin[t];
     }
 
     s.worker_begin.resize(n_workers + 1);

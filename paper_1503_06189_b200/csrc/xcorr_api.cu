@@ -30,7 +30,10 @@ struct xcorr_handle {
     int n_tiles = 0;                 // F * n_supertiles
     bool offdiag = false;            // N > 256: kernel variant with the column block and -Im plane
     size_t frame_bytes = 0, output_bytes = 0, acc_bytes = 0;
-    int32_t *acc = nullptr;          // device accumulator (layout.hpp)
+    int32_t *acc = nullptr;          // device accumulator slots (layout.hpp), one per work segment
+    int32_t *tile_slot_begin = nullptr;  // device, n_tiles + 1
+    int n_slots = 0;
+    bool clean = true;               // no frame since create / the last read: the next epilogue stores instead of adding
     int32_t *staging = nullptr;      // device packed triangle for host reads
     Segment *segments = nullptr;     // device
     int32_t *worker_begin = nullptr; // device
@@ -95,6 +98,7 @@ extern "C" void xcorr_destroy(xcorr_handle *h)
     cudaFree(h->staging);
     cudaFree(h->segments);
     cudaFree(h->worker_begin);
+    cudaFree(h->tile_slot_begin);
     delete h;
 }
 
@@ -121,7 +125,6 @@ extern "C" int xcorr_create(int n_inputs, int n_freq, int t_per_frame, xcorr_han
     h->output_bytes = (size_t)n_freq * ((size_t)n_inputs * (n_inputs + 1) / 2) * 8;
     const int nb = n_super(n_inputs);
     h->n_tiles = n_freq * n_supertiles(nb);
-    h->acc_bytes = (size_t)h->n_tiles * kAccElemsPerTile * sizeof(int32_t);
     h->offdiag = nb > 1;
     h->n_workers = prop.multiProcessorCount / 2;
     if (h->n_workers < 1) { delete h; return XCORR_EARCH; }
@@ -134,12 +137,18 @@ extern "C" int xcorr_create(int n_inputs, int n_freq, int t_per_frame, xcorr_han
     h->encode = (PFN_encodeTiled)fn;
 
     const Schedule sched = make_schedule(n_inputs, n_freq, t_per_frame, h->n_workers);
+    h->n_slots = (int)sched.segments.size();
+    h->acc_bytes = (size_t)h->n_slots * kAccElemsPerSlot * sizeof(int32_t);
     cudaError_t e;
     if ((e = cudaMalloc(&h->acc, h->acc_bytes)) != cudaSuccess) { h->last_cuda_error = e; return fail(XCORR_ENOMEM); }
     if ((e = cudaMalloc(&h->staging, h->output_bytes)) != cudaSuccess) { h->last_cuda_error = e; return fail(XCORR_ENOMEM); }
     if ((e = cudaMalloc(&h->segments, sizeof(Segment) * (sched.segments.size() + 1))) != cudaSuccess) return fail(XCORR_ENOMEM);
     if ((e = cudaMalloc(&h->worker_begin, sizeof(int32_t) * sched.worker_begin.size())) != cudaSuccess) return fail(XCORR_ENOMEM);
+    if ((e = cudaMalloc(&h->tile_slot_begin, sizeof(int32_t) * sched.tile_slot_begin.size())) != cudaSuccess) return fail(XCORR_ENOMEM);
     if (cudaMemset(h->acc, 0, h->acc_bytes) != cudaSuccess) return fail(XCORR_ECUDA);
+    if (cudaMemcpy(h->tile_slot_begin, sched.tile_slot_begin.data(), sizeof(int32_t) * sched.tile_slot_begin.size(),
+                   cudaMemcpyHostToDevice) != cudaSuccess)
+        return fail(XCORR_ECUDA);
     if (!sched.segments.empty() &&
         cudaMemcpy(h->segments, sched.segments.data(), sizeof(Segment) * sched.segments.size(), cudaMemcpyHostToDevice) != cudaSuccess)
         return fail(XCORR_ECUDA);
@@ -195,6 +204,7 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
     p.segments = h->segments;
     p.worker_begin = h->worker_begin;
     p.acc = h->acc;
+    p.first_frame = h->clean ? 1 : 0;
     p.n_inputs = h->n_inputs;
     p.n_freq = h->n_freq;
     p.n_time = h->n_time;
@@ -207,6 +217,7 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
     XC_CUDA(h, cudaGetLastError());
     h->launches += 1;
     h->samples_since_read += h->n_time;
+    h->clean = false;
     return XCORR_OK;
 }
 
@@ -223,11 +234,13 @@ extern "C" int xcorr_read(xcorr_handle *h, int32_t *upper_triangle_out, void *cu
     if (on_device && ((uintptr_t)upper_triangle_out & 15u) != 0) return XCORR_EINVAL;
     int32_t *dst = on_device ? upper_triangle_out : h->staging;
     const int nt = (h->n_inputs + 31) / 32;
-    finalize_kernel<<<dim3(nt, nt, h->n_freq), dim3(32, 8), 0, s>>>(h->acc, dst, h->n_inputs);
+    if (h->clean) XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, s));   // nothing integrated: the result is all zeros
+    finalize_kernel<<<dim3(nt, nt, h->n_freq), 256, 0, s>>>(h->acc, h->tile_slot_begin, dst, h->n_inputs);
     XC_CUDA(h, cudaGetLastError());
     h->launches += 1;
-    XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, s));      // ends the integration
+    // ends the integration: no clearing pass -- the next frame's epilogue overwrites its slots (first_frame)
     h->samples_since_read = 0;
+    h->clean = true;
     if (!on_device) {
         XC_CUDA(h, cudaMemcpyAsync(upper_triangle_out, h->staging, h->output_bytes, cudaMemcpyDeviceToHost, s));
         XC_CUDA(h, cudaStreamSynchronize(s));
@@ -323,8 +336,8 @@ extern "C" int xcorr_debug_schedule(int n_inputs, int n_freq, int t_per_frame, i
         if (n > max_segments) return XCORR_EINVAL;
         for (int k = 0; k < n; ++k) {
             const Segment &g = sched.segments[k];
-            int32_t *o = segments_out + 6 * k;
-            o[0] = g.f; o[1] = g.I; o[2] = g.J; o[3] = g.stage_begin; o[4] = g.stage_end; o[5] = g.tile;
+            int32_t *o = segments_out + 7 * k;
+            o[0] = g.f; o[1] = g.I; o[2] = g.J; o[3] = g.stage_begin; o[4] = g.stage_end; o[5] = g.tile; o[6] = g.slot;
         }
         for (int w = 0; w <= n_workers; ++w) worker_begin_out[w] = sched.worker_begin[w];
     }
@@ -338,10 +351,12 @@ extern "C" int xcorr_debug_process_simt(xcorr_handle *h, const void *packed_fram
     int rc = check_process_args(h, packed_frame_dev);
     if (rc != XCORR_OK) return rc;
     const int blocks = h->n_tiles * 2 * (kBlock / 8);
-    simt_reference_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const uint8_t *)packed_frame_dev, h->acc, h->n_inputs,
-                                                                            h->n_freq, h->n_time);
+    if (h->clean) XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, (cudaStream_t)cuda_stream));
+    simt_reference_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const uint8_t *)packed_frame_dev, h->acc, h->tile_slot_begin,
+                                                                            h->n_inputs, h->n_freq, h->n_time);
     XC_CUDA(h, cudaGetLastError());
     h->launches += 1;
     h->samples_since_read += h->n_time;
+    h->clean = false;
     return XCORR_OK;
 }

@@ -6,7 +6,7 @@
 //   a3  one thread issues 2-CTA tcgen05.mma kind::i8 (M = 256 over the CTA pair, N = 256, K = 32) with
 //       both operands MN-major straight from those planes; int32 accumulators stay in TMEM (512 columns)
 //       for the whole time range of the work segment
-//   a4  epilogue warps tcgen05.ld the accumulators and red.add them into the device accumulator
+//   a4  epilogue warps tcgen05.ld the accumulators and add them into this segment's accumulator slot (no atomics)
 //
 // Complex product from stacked real GEMMs (BASELINE.json:north_star (b)); h = Re plane, l = Im plane:
 //   diagonal super-tile (I == J):   R += h h^T ; R += l l^T ; Q += l h^T      (Im V = Q - Q^T, formed at read)
@@ -61,7 +61,8 @@ constexpr int kNumEpiWarps = 4;
 struct KernelParams {
     const Segment *segments;       // device
     const int32_t *worker_begin;   // device, n_workers + 1
-    int32_t *acc;                  // device accumulator, layout.hpp
+    int32_t *acc;                  // device accumulator slots, layout.hpp
+    int first_frame;               // 1: first frame of an integration -> epilogue stores; 0: load-add-store
     int n_inputs;
     int n_freq;
     int n_time;
@@ -275,27 +276,37 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             const int row0 = (int)(rank * kBlock + quarter * 32);             // first row of this warp inside the super-block
             const int rows_valid = p.n_inputs - seg.I * kSuper - row0;         // rows of this warp that are real inputs
             const int cols_valid = min(kSuper, p.n_inputs - seg.J * kSuper);   // columns that are real inputs
-            int32_t *acc_cta = p.acc + ((size_t)seg.tile * 2 + rank) * (size_t)kAccElemsPerCta + quarter * 32 + lane;
+            // this segment's own slot: [r][col/4][row][4] int32 -> one warp's 16-byte accesses are 512 B contiguous
+            int32_t *slot_cta = p.acc + ((size_t)seg.slot * 2 + rank) * (size_t)kAccElemsPerCta + (size_t)(quarter * 32 + lane) * 4;
+#ifdef XC_DEBUG_SKIP_EPI
+            if (false) {
+#else
             if (rows_valid > 0) {
+#endif
                 // R columns: on a diagonal super-tile only j >= i is ever read -> start at this warp's first row
                 const int r_begin = (seg.I == seg.J) ? row0 : 0;
-                for (int c = r_begin; c < cols_valid; c += 32) {
+                const int n_chunks_r = (cols_valid - r_begin + 31) / 32;      // may be <= 0
+                const int n_chunks_q = (cols_valid + 31) / 32;
+                for (int ch = 0; ch < max(n_chunks_r, 0) + n_chunks_q; ++ch) {
+                    const int col = (ch < n_chunks_r) ? (r_begin + 32 * ch) : (256 + 32 * (ch - max(n_chunks_r, 0)));
                     uint32_t v[32];
-                    ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + (uint32_t)c, v);
+                    ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + (uint32_t)col, v);
                     ptx::tmem_wait_ld();
-#ifndef XC_DEBUG_SKIP_RED
+                    int32_t *dst = slot_cta + (size_t)(col >> 2) * (kBlock * 4);
+                    if (p.first_frame) {
 #pragma unroll
-                    for (int k = 0; k < 32; ++k) ptx::red_add_s32(acc_cta + (size_t)(c + k) * kBlock, (int32_t)v[k]);
-#endif
-                }
-                for (int c = 0; c < cols_valid; c += 32) {
-                    uint32_t v[32];
-                    ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + 256u + (uint32_t)c, v);
-                    ptx::tmem_wait_ld();
-#ifndef XC_DEBUG_SKIP_RED
+                        for (int g = 0; g < 8; ++g)
+                            ptx::st_global_v4(dst + g * (kBlock * 4), (int32_t)v[4 * g], (int32_t)v[4 * g + 1], (int32_t)v[4 * g + 2],
+                                              (int32_t)v[4 * g + 3]);
+                    } else {
+                        int4 old[8];
 #pragma unroll
-                    for (int k = 0; k < 32; ++k) ptx::red_add_s32(acc_cta + (size_t)(256 + c + k) * kBlock, (int32_t)v[k]);
-#endif
+                        for (int g = 0; g < 8; ++g) old[g] = ptx::ld_global_v4(dst + g * (kBlock * 4));
+#pragma unroll
+                        for (int g = 0; g < 8; ++g)
+                            ptx::st_global_v4(dst + g * (kBlock * 4), old[g].x + (int32_t)v[4 * g], old[g].y + (int32_t)v[4 * g + 1],
+                                              old[g].z + (int32_t)v[4 * g + 2], old[g].w + (int32_t)v[4 * g + 3]);
+                    }
                 }
             }
             ptx::tc_fence_before_sync();

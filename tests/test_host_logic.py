@@ -21,12 +21,16 @@ def _check(n, f, t, workers):
     load = np.zeros(workers, dtype=np.int64)
     for w in range(workers):
         for k in range(wb[w], wb[w + 1]):
-            ff, I, J, s0, s1, tile = seg[k]
+            ff, I, J, s0, s1, tile, slot = seg[k]
             assert 0 <= ff < f and 0 <= I <= J < nb and 0 <= s0 < s1 <= n_stage
             assert tile == ff * nst + I * (2 * nb - I + 1) // 2 + (J - I)
             cover[tile, s0:s1] += 1
             load[w] += (3 if I == J else 4) * (s1 - s0)
     assert (cover == 1).all(), "every (super-tile, stage) must be processed exactly once"
+    # every segment owns its own accumulator slot; a tile's slots are contiguous and ordered by time
+    assert sorted(seg[:, 6].tolist()) == list(range(len(seg)))
+    order = np.lexsort((seg[:, 3], seg[:, 5]))
+    assert (seg[order, 6] == np.arange(len(seg))).all()
     return load, n_stage
 
 
