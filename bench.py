@@ -99,7 +99,7 @@ def oracle_sample(cfg: wl.Config, seconds_hint: float = 12.0):
     import oracle
     oracle.build()
     cores = oracle.threads()
-    n_ch = max(1, min(cfg.n_freq, 2 * cores if cfg.n_inputs <= 256 else 1))
+    n_ch = max(1, min(cfg.n_freq, 8 * cores if cfg.n_inputs <= 256 else 1))
     t_samp = cfg.n_time if cfg.n_inputs <= 512 else min(cfg.n_time, 2048)
     fr = wl.make_frame(cfg.kind, cfg.n_inputs, n_ch, t_samp, cfg.seed)
     t0 = time.perf_counter()
@@ -140,7 +140,7 @@ def run_reference(args, cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C2", choices=sorted(wl.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -153,6 +153,7 @@ def main():
 
     import torch
     import paper_1503_06189_b200 as xb
+    from paper_1503_06189_b200 import replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -214,10 +215,7 @@ def main():
     kern_ms = [a.elapsed_time(b) for a, b in evs]
     clocks = sampler.stop()
 
-    if dist is not None:
-        tt = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+    total_ms = replicas.max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / steps
     bits_per_frame = 8.0 * cfg.frame_bytes
     value = world * bits_per_frame / (ms_per_step * 1e-3) / 1e9
@@ -253,10 +251,7 @@ def main():
             s.read(out_host)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            tt = torch.tensor([dt], device="cuda")
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt.item())
+        dt = replicas.max_over_ranks(dt, dist, "cuda")
         e2e = {"value": world * bits_per_frame * n_e2e / dt / 1e9, "unit": "Gb/s", "h2d_bytes_per_step": cfg.frame_bytes,
                "d2h_bytes_per_step": cfg.output_bytes, "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3,
                "api": "xcorr_stream_submit(pinned host frame) + xcorr_stream_read(pinned host out)"}
