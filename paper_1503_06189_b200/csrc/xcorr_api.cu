@@ -209,11 +209,11 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
     p.n_freq = h->n_freq;
     p.n_time = h->n_time;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    const dim3 grid(2 * h->n_workers), block(kThreads);
+    const dim3 grid(2 * h->n_workers);
     if (h->offdiag)
-        xengine_kernel<true><<<grid, block, KernelCfg<true>::kSmemBytes, s>>>(map, p);
+        xengine_kernel<true><<<grid, KernelCfg<true>::kThreads, KernelCfg<true>::kSmemBytes, s>>>(map, p);
     else
-        xengine_kernel<false><<<grid, block, KernelCfg<false>::kSmemBytes, s>>>(map, p);
+        xengine_kernel<false><<<grid, KernelCfg<false>::kThreads, KernelCfg<false>::kSmemBytes, s>>>(map, p);
     XC_CUDA(h, cudaGetLastError());
     h->launches += 1;
     h->samples_since_read += h->n_time;

@@ -45,17 +45,24 @@ struct KernelCfg {
 #endif
     static constexpr int kPackedStages = kOffDiag ? 3 : XC_PACKED_STAGES_DIAG;
     static constexpr int kPlaneStages = kOffDiag ? 3 : XC_PLANE_STAGES_DIAG;
+#ifndef XC_UNPACK_WARPS_OFFDIAG
+#define XC_UNPACK_WARPS_OFFDIAG 8
+#endif
+#ifndef XC_UNPACK_WARPS_DIAG
+#define XC_UNPACK_WARPS_DIAG 8
+#endif
+    static constexpr int kUnpackWarps = kOffDiag ? XC_UNPACK_WARPS_OFFDIAG : XC_UNPACK_WARPS_DIAG;   // multiple of 4
+    static constexpr int kUnpackThreads = kUnpackWarps * 32;
+    static constexpr int kWarpEpi0 = 4 + kUnpackWarps;             // epilogue warps: warp % 4 == TMEM lane quarter
+    static constexpr int kThreads = (4 + kUnpackWarps + 4) * 32;
     static constexpr int kSmemData = kPackedStages * kPackedStageBytes + kPlaneStages * kPlaneStageBytes;
     static constexpr int kSmemBytes = kSmemData + 1024 /*align slack*/ + 1024 /*barriers*/;
 };
 
-constexpr int kThreads = 384;          // 12 warps
 constexpr int kWarpTma = 0;
 constexpr int kWarpMma = 1;
 constexpr int kWarpTmem = 2;
-constexpr int kWarpUnpack0 = 4;        // warps 4..7
-constexpr int kNumUnpackWarps = 4;
-constexpr int kWarpEpi0 = 8;           // warps 8..11 (warp % 4 == TMEM lane quarter)
+constexpr int kWarpUnpack0 = 4;        // unpack warps 4 .. 4 + Cfg::kUnpackWarps - 1, then 4 epilogue warps
 constexpr int kNumEpiWarps = 4;
 
 struct KernelParams {
@@ -92,7 +99,7 @@ __device__ __forceinline__ uint32_t negate4(uint32_t y)
 // the kernel
 // ------------------------------------------------------------------------------------------------
 template <bool kOffDiag>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(KernelCfg<kOffDiag>::kThreads, 1)
 xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams p)
 {
     using Cfg = KernelCfg<kOffDiag>;
@@ -120,10 +127,10 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     if (warp == kWarpMma && lane == 0) {
         for (int s = 0; s < Cfg::kPackedStages; ++s) {
             ptx::mbar_init(bar_pk_full(s), 1);                    // TMA producer's arrive.expect_tx
-            ptx::mbar_init(bar_pk_empty(s), kNumUnpackWarps);     // one arrive per unpack warp
+            ptx::mbar_init(bar_pk_empty(s), Cfg::kUnpackWarps);     // one arrive per unpack warp
         }
         for (int s = 0; s < Cfg::kPlaneStages; ++s) {
-            ptx::mbar_init(bar_pl_full(s), 2 * kNumUnpackWarps);  // unpack warps of BOTH CTAs (used in the leader only)
+            ptx::mbar_init(bar_pl_full(s), 2 * Cfg::kUnpackWarps);  // unpack warps of BOTH CTAs (used in the leader only)
             ptx::mbar_init(bar_pl_empty(s), 1);                   // tcgen05.commit (multicast to both CTAs)
         }
         ptx::mbar_init(bar_acc_full, 1);                          // tcgen05.commit (multicast)
@@ -209,9 +216,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 ptx::mma_commit<2>(bar_acc_full, 0x3);             // accumulators complete (both CTAs)
             }
         }
-    } else if (warp >= kWarpUnpack0 && warp < kWarpUnpack0 + kNumUnpackWarps) {
+    } else if (warp >= kWarpUnpack0 && warp < (uint32_t)Cfg::kWarpEpi0) {
         // ===================================================== a2: unpack warps
-        const uint32_t tid = threadIdx.x - kWarpUnpack0 * 32;     // 0..127
+        const uint32_t tid = threadIdx.x - kWarpUnpack0 * 32;     // 0 .. kUnpackThreads-1
         const uint32_t pl_full_leader = ptx::mapa(bar_base, 0) + (bar_pl_full(0) - bar_base);
         uint32_t it = 0;
         for (int sg = seg_begin; sg < seg_end; ++sg) {
@@ -225,8 +232,8 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 const uint32_t src = smem_packed + pslot * Cfg::kPackedStageBytes;
                 const uint32_t dst = smem_planes + lslot * Cfg::kPlaneStageBytes;
 #pragma unroll
-                for (int q = 0; q < Cfg::kPlaneBytes / (128 * 16); ++q) {
-                    const uint32_t o = (uint32_t)(q * 128 + tid) * 16u;
+                for (int q = 0; q < Cfg::kPlaneBytes / (Cfg::kUnpackThreads * 16); ++q) {
+                    const uint32_t o = (uint32_t)(q * Cfg::kUnpackThreads + tid) * 16u;
                     uint32_t w0, w1, w2, w3;
                     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3) : "r"(src + o));
                     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + o), "r"(unpack_re4(w0)), "r"(unpack_re4(w1)),
@@ -238,8 +245,8 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 }
                 if (off) {
 #pragma unroll
-                    for (int q = 0; q < Cfg::kPlaneBytes / (128 * 16); ++q) {
-                        const uint32_t o = (uint32_t)(q * 128 + tid) * 16u;
+                    for (int q = 0; q < Cfg::kPlaneBytes / (Cfg::kUnpackThreads * 16); ++q) {
+                        const uint32_t o = (uint32_t)(q * Cfg::kUnpackThreads + tid) * 16u;
                         uint32_t w0, w1, w2, w3;
                         asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
                                      : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3)
@@ -264,7 +271,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 }
             }
         }
-    } else if (warp >= kWarpEpi0) {
+    } else if (warp >= (uint32_t)Cfg::kWarpEpi0) {
         // ===================================================== a4: epilogue warps
         const uint32_t quarter = warp & 3u;                      // TMEM lanes [32*quarter, 32*quarter+32)
         const uint32_t acc_empty_leader = ptx::mapa(bar_acc_empty, 0);
