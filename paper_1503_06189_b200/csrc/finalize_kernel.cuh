@@ -4,7 +4,16 @@
 // A slot is [r][col/4][row][4] (row = TMEM lane fast), the output is row-major in (i, j).  Each block turns one
 // 32 x 32 patch around through shared memory so that both sides are coalesced: 16-byte vector reads along the row
 // index, 8-byte (re, im) writes along j.  The slots of a super-tile (one per work segment that summed part of
-// its time range) are added here.  On diagonal super-tiles Im V[i,j] = X[i,j] - X[j,i] (layout.hpp).
+// its time range) are added here, and the operand offsets are removed (layout.hpp "OFFSET OPERANDS"): with
+// h = h' - 8, l = l' - 8, the column sums sh_n = sum_t h'_n, sl_n = sum_t l'_n of the tile's sum slots and
+// T' = the number of (zero-padded) samples the tensor path has integrated,
+//
+//   Re V[i,j] = R'[i,j] - 8 (sh_i + sl_i + sh_j + sl_j) + 128 T'
+//   Im V[i,j] = Q'[i,j] - Q'[j,i] + 8 (sh_i - sl_i) - 8 (sh_j - sl_j)               on diagonal super-tiles (I == J)
+//   Im V[i,j] = Q'[i,j] - 7 sh_i - 8 sl_i - 8 sh_j + 8 sl_j                         for I < J, where Q' holds
+//               sum l'_i h'_j + h'_i (15 - l'_j)
+//
+// exactly, modulo 2^32 (unsigned arithmetic below; the true values fit int32 by the overflow guard).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -14,26 +23,28 @@
 namespace xc {
 
 // sum over the tile's slots of the 4 consecutive columns [col4*4, col4*4+4) of row `row`, CTA half r
-__device__ __forceinline__ int4 slot_sum_v4(const int32_t *__restrict__ acc, int slot_begin, int slot_end, int r, int col4, int row)
+__device__ __forceinline__ uint4 slot_sum_v4(const int32_t *__restrict__ acc, int slot_begin, int slot_end, int r, int col4, int row)
 {
-    int4 s = make_int4(0, 0, 0, 0);
+    uint4 s = make_uint4(0, 0, 0, 0);
     for (int sl = slot_begin; sl < slot_end; ++sl) {
-        const int4 v = *reinterpret_cast<const int4 *>(acc + (size_t)sl * kAccElemsPerSlot + (size_t)r * kAccElemsPerCta +
-                                                       ((size_t)col4 * kBlock + row) * 4);
+        const uint4 v = *reinterpret_cast<const uint4 *>(acc + (size_t)sl * kAccElemsPerSlot + (size_t)r * kAccElemsPerCta +
+                                                         ((size_t)col4 * kBlock + row) * 4);
         s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
     }
     return s;
 }
 
 // grid (nt, nt, F), nt = ceil(N / 32); block 256 threads
-__global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict__ acc, const int32_t *__restrict__ tile_slot_begin,
-                                                        int32_t *__restrict__ out, int n_inputs)
+__global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict__ acc, const int32_t *__restrict__ sums,
+                                                        const int32_t *__restrict__ tile_slot_begin, int32_t *__restrict__ out, int n_inputs,
+                                                        uint32_t offset_samples)
 {
     const int bj = blockIdx.x, bi = blockIdx.y, f = blockIdx.z;
     if (bj < bi) return;
-    __shared__ int32_t sR[32][33];   // [col][row]
-    __shared__ int32_t sQ[32][33];   // [col][row]
-    __shared__ int32_t sX[32][33];   // [row j][col i] of the transposed patch (diagonal super-tiles only)
+    __shared__ uint32_t sR[32][33];   // [col][row]
+    __shared__ uint32_t sQ[32][33];   // [col][row]
+    __shared__ uint32_t sX[32][33];   // [row j][col i] of the transposed patch (diagonal super-tiles only)
+    __shared__ uint32_t sS[4][32];    // column sums: [0] sh_i [1] sl_i (rows of the patch)  [2] sh_j [3] sl_j (columns)
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;   // ty in 0..7
     const int nb = n_super(n_inputs), nst = n_supertiles(nb);
     const int i0 = bi * 32, j0 = bj * 32;
@@ -47,27 +58,40 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
         const int il = (i0 % kSuper) + tx;            // row inside the super-block
         const int r = il / kBlock, row = il % kBlock;
         const int c4 = ((j0 % kSuper) >> 2) + ty;     // column group inside the super-block
-        const int4 vr = slot_sum_v4(acc, sb, se, r, c4, row);
-        const int4 vq = slot_sum_v4(acc, sb, se, r, 64 + c4, row);
+        const uint4 vr = slot_sum_v4(acc, sb, se, r, c4, row);
+        const uint4 vq = slot_sum_v4(acc, sb, se, r, 64 + c4, row);
         sR[4 * ty + 0][tx] = vr.x; sR[4 * ty + 1][tx] = vr.y; sR[4 * ty + 2][tx] = vr.z; sR[4 * ty + 3][tx] = vr.w;
         sQ[4 * ty + 0][tx] = vq.x; sQ[4 * ty + 1][tx] = vq.y; sQ[4 * ty + 2][tx] = vq.z; sQ[4 * ty + 3][tx] = vq.w;
         if (diag_super) {
             // X[j][i] for rows j in [j0, j0+32), columns i in [i0, i0+32)
             const int jl = (j0 % kSuper) + tx;
-            const int4 vx = slot_sum_v4(acc, sb, se, jl / kBlock, 64 + ((i0 % kSuper) >> 2) + ty, jl % kBlock);
+            const uint4 vx = slot_sum_v4(acc, sb, se, jl / kBlock, 64 + ((i0 % kSuper) >> 2) + ty, jl % kBlock);
             sX[tx][4 * ty + 0] = vx.x; sX[tx][4 * ty + 1] = vx.y; sX[tx][4 * ty + 2] = vx.z; sX[tx][4 * ty + 3] = vx.w;
+        }
+        if (ty < 4) {
+            // ty 0,1: sh, sl of row input i0 + tx (A block of its CTA half); ty 2,3: of column input j0 + tx
+            // (A block again on a diagonal super-tile, the B block for I < J)
+            const int nl = ((ty < 2) ? (i0 % kSuper) : (j0 % kSuper)) + tx;
+            const int plane = (ty & 1) + ((ty >= 2 && !diag_super) ? 2 : 0);
+            uint32_t v = 0;
+            for (int sl = sb; sl < se; ++sl)
+                v += (uint32_t)sums[(size_t)sl * kSumElemsPerSlot + (size_t)(nl / kBlock) * kSumElemsPerCta + plane * kBlock + (nl % kBlock)];
+            sS[ty][tx] = v;
         }
     }
     __syncthreads();
     // phase 2: tx <-> column j0 + tx, one output row per ty step: 8-byte (re, im) writes, 256 B contiguous per warp
     const long long P = (long long)n_inputs * (n_inputs + 1) / 2;
+    const uint32_t shj = sS[2][tx], slj = sS[3][tx];
     for (int ic = ty; ic < 32; ic += 8) {
         const int i = i0 + ic, j = j0 + tx;
         if (j < n_inputs && i <= j) {
-            const int32_t re = sR[tx][ic];
-            int32_t im = sQ[tx][ic];
-            if (diag_super) im = (i == j) ? 0 : im - sX[tx][ic];
-            *reinterpret_cast<int2 *>(out + ((long long)f * P + pair_index(n_inputs, i, j)) * 2) = make_int2(re, im);
+            const uint32_t shi = sS[0][ic], sli = sS[1][ic];
+            const uint32_t re = sR[tx][ic] - 8u * (shi + sli + shj + slj) + 128u * offset_samples;
+            uint32_t im;
+            if (diag_super) im = (i == j) ? 0u : sQ[tx][ic] - sX[tx][ic] + 8u * (shi - sli) - 8u * (shj - slj);
+            else im = sQ[tx][ic] - 7u * shi - 8u * sli - 8u * shj + 8u * slj;
+            *reinterpret_cast<int2 *>(out + ((long long)f * P + pair_index(n_inputs, i, j)) * 2) = make_int2((int32_t)re, (int32_t)im);
         }
     }
 }

@@ -20,6 +20,19 @@
 //
 // Lower-triangle R entries of diagonal super-tiles and anything with i >= N or j >= N are never read
 // (and mostly never written).
+//
+// OFFSET OPERANDS.  The tensor core is fed x' = x + 8 in [0, 15] (h' = h + 8, l' = l + 8; and the complement
+// 15 - l' where a negated operand is needed) instead of the sign-extended int8 value: the upper nibble of every
+// operand byte is then constant zero, which measurably lowers the switching power of the MMA datapath (the part is
+// power-limited).  The slots therefore hold the OFFSET sums
+//     R'[i,j] = sum h'_i h'_j + l'_i l'_j          Q'[i,j] = sum l'_i h'_j  ( + h'_i (15 - l'_j) for I < J )
+// and every segment also owns a row of per-input column sums over its time range ("sum slot"):
+//
+//   sums[slot][r][plane][row]   int32,  plane 0: sum_t h'   1: sum_t l'   of input 256*I + 128*r + row   (A block)
+//                                       plane 2: sum_t h'   3: sum_t l'   of input 256*J + 128*r + row   (B block, I < J)
+//
+// xcorr_read removes the offsets exactly (finalize_kernel.cuh); all arithmetic is modulo 2^32 and the final values fit
+// int32 by the overflow guard, so intermediate wrap-around of R', Q' is harmless (tcgen05 kind::i8 accumulators wrap).
 #pragma once
 #include <cstdint>
 
@@ -30,6 +43,9 @@ constexpr int kSuper = 256;        // inputs per super-block (CTA pair)
 constexpr int kAccCols = 512;      // TMEM columns per CTA: 256 R + 256 Q
 constexpr int kAccElemsPerCta = kAccCols * kBlock;          // 65536 int32
 constexpr int kAccElemsPerSlot = 2 * kAccElemsPerCta;        // 131072 int32 = 512 KiB
+constexpr int kSumPlanes = 4;                                // h'_A, l'_A, h'_B, l'_B
+constexpr int kSumElemsPerCta = kSumPlanes * kBlock;          // 512 int32
+constexpr int kSumElemsPerSlot = 2 * kSumElemsPerCta;         // 1024 int32 = 4 KiB
 
 __host__ __device__ inline int n_super(int n_inputs) { return (n_inputs + kSuper - 1) / kSuper; }
 __host__ __device__ inline int n_supertiles(int nb) { return nb * (nb + 1) / 2; }

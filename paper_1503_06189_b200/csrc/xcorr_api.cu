@@ -31,6 +31,9 @@ struct xcorr_handle {
     bool offdiag = false;            // N > 256: kernel variant with the column block and -Im plane
     size_t frame_bytes = 0, output_bytes = 0, acc_bytes = 0;
     int32_t *acc = nullptr;          // device accumulator slots (layout.hpp), one per work segment
+    int32_t *sums = nullptr;         // device column-sum slots (layout.hpp), one per work segment
+    size_t sums_bytes = 0;
+    unsigned long long offset_samples = 0;  // zero-padded samples the tensor path integrated since the last read (offset removal)
     int32_t *tile_slot_begin = nullptr;  // device, n_tiles + 1
     int n_slots = 0;
     bool clean = true;               // no frame since create / the last read: the next epilogue stores instead of adding
@@ -95,6 +98,7 @@ extern "C" void xcorr_destroy(xcorr_handle *h)
     cudaSetDevice(h->device);
     cudaDeviceSynchronize();
     cudaFree(h->acc);
+    cudaFree(h->sums);
     cudaFree(h->staging);
     cudaFree(h->segments);
     cudaFree(h->worker_begin);
@@ -141,6 +145,9 @@ extern "C" int xcorr_create(int n_inputs, int n_freq, int t_per_frame, xcorr_han
     h->acc_bytes = (size_t)h->n_slots * kAccElemsPerSlot * sizeof(int32_t);
     cudaError_t e;
     if ((e = cudaMalloc(&h->acc, h->acc_bytes)) != cudaSuccess) { h->last_cuda_error = e; return fail(XCORR_ENOMEM); }
+    h->sums_bytes = (size_t)h->n_slots * kSumElemsPerSlot * sizeof(int32_t);
+    if ((e = cudaMalloc(&h->sums, h->sums_bytes)) != cudaSuccess) { h->last_cuda_error = e; return fail(XCORR_ENOMEM); }
+    if (cudaMemset(h->sums, 0, h->sums_bytes) != cudaSuccess) return fail(XCORR_ECUDA);
     if ((e = cudaMalloc(&h->staging, h->output_bytes)) != cudaSuccess) { h->last_cuda_error = e; return fail(XCORR_ENOMEM); }
     if ((e = cudaMalloc(&h->segments, sizeof(Segment) * (sched.segments.size() + 1))) != cudaSuccess) return fail(XCORR_ENOMEM);
     if ((e = cudaMalloc(&h->worker_begin, sizeof(int32_t) * sched.worker_begin.size())) != cudaSuccess) return fail(XCORR_ENOMEM);
@@ -204,6 +211,7 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
     p.segments = h->segments;
     p.worker_begin = h->worker_begin;
     p.acc = h->acc;
+    p.sums = h->sums;
     p.first_frame = h->clean ? 1 : 0;
     p.n_inputs = h->n_inputs;
     p.n_freq = h->n_freq;
@@ -217,6 +225,7 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
     XC_CUDA(h, cudaGetLastError());
     h->launches += 1;
     h->samples_since_read += h->n_time;
+    h->offset_samples += (unsigned long long)((h->n_time + kStageT - 1) / kStageT) * kStageT;   // TMA zero fill = samples of value 0
     h->clean = false;
     return XCORR_OK;
 }
@@ -234,12 +243,17 @@ extern "C" int xcorr_read(xcorr_handle *h, int32_t *upper_triangle_out, void *cu
     if (on_device && ((uintptr_t)upper_triangle_out & 15u) != 0) return XCORR_EINVAL;
     int32_t *dst = on_device ? upper_triangle_out : h->staging;
     const int nt = (h->n_inputs + 31) / 32;
-    if (h->clean) XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, s));   // nothing integrated: the result is all zeros
-    finalize_kernel<<<dim3(nt, nt, h->n_freq), 256, 0, s>>>(h->acc, h->tile_slot_begin, dst, h->n_inputs);
+    if (h->clean) {   // nothing integrated: the result is all zeros
+        XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, s));
+        XC_CUDA(h, cudaMemsetAsync(h->sums, 0, h->sums_bytes, s));
+    }
+    finalize_kernel<<<dim3(nt, nt, h->n_freq), 256, 0, s>>>(h->acc, h->sums, h->tile_slot_begin, dst, h->n_inputs,
+                                                            (uint32_t)h->offset_samples);
     XC_CUDA(h, cudaGetLastError());
     h->launches += 1;
     // ends the integration: no clearing pass -- the next frame's epilogue overwrites its slots (first_frame)
     h->samples_since_read = 0;
+    h->offset_samples = 0;
     h->clean = true;
     if (!on_device) {
         XC_CUDA(h, cudaMemcpyAsync(upper_triangle_out, h->staging, h->output_bytes, cudaMemcpyDeviceToHost, s));
@@ -351,7 +365,10 @@ extern "C" int xcorr_debug_process_simt(xcorr_handle *h, const void *packed_fram
     int rc = check_process_args(h, packed_frame_dev);
     if (rc != XCORR_OK) return rc;
     const int blocks = h->n_tiles * 2 * (kBlock / 8);
-    if (h->clean) XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, (cudaStream_t)cuda_stream));
+    if (h->clean) {
+        XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, (cudaStream_t)cuda_stream));
+        XC_CUDA(h, cudaMemsetAsync(h->sums, 0, h->sums_bytes, (cudaStream_t)cuda_stream));
+    }
     simt_reference_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const uint8_t *)packed_frame_dev, h->acc, h->tile_slot_begin,
                                                                             h->n_inputs, h->n_freq, h->n_time);
     XC_CUDA(h, cudaGetLastError());

@@ -2,16 +2,20 @@
 //
 //   a1  TMA stages packed bytes  frame[t][f][128 inputs]  as 128-byte rows (SWIZZLE_128B) into smem
 //   a2  unpack warps split each byte into int8 Re / Im planes (same swizzled 128-byte-row layout, so
-//       the unpack is purely element-wise and never looks at the swizzle)
+//       the unpack is purely element-wise and never looks at the swizzle).  The planes hold the OFFSET values
+//       h' = Re + 8, l' = Im + 8 in [0, 15] (layout.hpp "OFFSET OPERANDS": constant-zero upper nibbles cut the
+//       MMA datapath's switching power, and the part is power-limited); the same warps keep per-input column
+//       sums of h', l' so that xcorr_read can remove the offsets exactly
 //   a3  one thread issues 2-CTA tcgen05.mma kind::i8 (M = 256 over the CTA pair, N = 256, K = 32) with
 //       both operands MN-major straight from those planes; int32 accumulators stay in TMEM (512 columns)
 //       for the whole time range of the work segment
 //   a4  epilogue warps tcgen05.ld the accumulators and add them into this segment's accumulator slot (no atomics)
 //
-// Complex product from stacked real GEMMs (BASELINE.json:north_star (b)); h = Re plane, l = Im plane:
+// Complex product from stacked real GEMMs (BASELINE.json:north_star (b)); h = Re plane, l = Im plane (offset values):
 //   diagonal super-tile (I == J):   R += h h^T ; R += l l^T ; Q += l h^T      (Im V = Q - Q^T, formed at read)
-//   off-diagonal        (I <  J):   R += h_I h_J^T ; R += l_I l_J^T ; Q += l_I h_J^T ; Q += h_I (-l_J)^T
-// Integer MMAs have no operand-negate bit, hence the explicit -l_J plane for I < J.
+//   off-diagonal        (I <  J):   R += h_I h_J^T ; R += l_I l_J^T ; Q += l_I h_J^T ; Q += h_I (15 - l_J)^T
+// Integer MMAs have no operand-negate bit, hence the explicit complement plane 15 - l'_J for I < J (the constant
+// 15 sum h'_I it adds is removed at read together with the offsets).
 //
 // One cluster = CTA pair = one "worker" of schedule.hpp; CTA rank r owns inputs [128r, 128r+128) of the
 // row super-block (A operand, TMEM lanes) and of the column super-block (its half of the B operand).
@@ -26,6 +30,20 @@
 
 namespace xc {
 
+// Optional stall accounting (development builds only, -DXC_PROFILE): per-CTA cycle counters of where each role waits.
+#ifdef XC_PROFILE
+__device__ unsigned long long g_prof[1024][16];
+#define XC_PROF_DECL(v) long long v = 0
+#define XC_PROF_BEGIN(v) const long long v##_t0 = clock64()
+#define XC_PROF_END(v) v += clock64() - v##_t0
+#define XC_PROF_STORE(idx, v) g_prof[blockIdx.x][idx] = (unsigned long long)(v)
+#else
+#define XC_PROF_DECL(v)
+#define XC_PROF_BEGIN(v)
+#define XC_PROF_END(v)
+#define XC_PROF_STORE(idx, v)
+#endif
+
 // ------------------------------------------------------------------------------------------------
 // compile-time configuration
 // ------------------------------------------------------------------------------------------------
@@ -34,7 +52,7 @@ struct KernelCfg {
     static constexpr int kRowBytes = 128;                          // one t-row of one 128-input block
     static constexpr int kPlaneBytes = kStageT * kRowBytes;        // 8 KiB: one plane (or packed block) per stage
     static constexpr int kPackedBlocks = kOffDiag ? 2 : 1;         // A block (+ B block when I < J)
-    static constexpr int kPlanes = kOffDiag ? 5 : 2;               // h_a l_a [h_b l_b -l_b]
+    static constexpr int kPlanes = kOffDiag ? 5 : 2;               // h_a l_a [h_b l_b 15-l_b]
     static constexpr int kPackedStageBytes = kPackedBlocks * kPlaneBytes;
     static constexpr int kPlaneStageBytes = kPlanes * kPlaneBytes;
 #ifndef XC_PACKED_STAGES_DIAG
@@ -55,8 +73,17 @@ struct KernelCfg {
     static constexpr int kUnpackThreads = kUnpackWarps * 32;
     static constexpr int kWarpEpi0 = 4 + kUnpackWarps;             // epilogue warps: warp % 4 == TMEM lane quarter
     static constexpr int kThreads = (4 + kUnpackWarps + 4) * 32;
-    static constexpr int kSmemData = kPackedStages * kPackedStageBytes + kPlaneStages * kPlaneStageBytes;
+    static constexpr int kSumPlanes = 2 * kPackedBlocks;           // column sums kept by the unpack warps: h'_a l'_a [h'_b l'_b]
+    static constexpr int kSumScratch = kUnpackThreads * 32;        // cross-thread reduction of the column sums (8 KiB)
+    static constexpr int kSmemData = kPackedStages * kPackedStageBytes + kPlaneStages * kPlaneStageBytes + kSumScratch;
     static constexpr int kSmemBytes = kSmemData + 1024 /*align slack*/ + 1024 /*barriers*/;
+    // column sums: a thread sees kRowsPerStage rows of its 16 inputs per stage; byte lanes hold 17 rows of values <= 15,
+    // 16-bit lanes 4369 rows
+    static constexpr int kRowsPerStage = kPlaneBytes / (kUnpackThreads * 16);
+    static constexpr int kWidenStages = 16 / kRowsPerStage;
+    static constexpr int kFlushStages = 4096 / kRowsPerStage;
+    static_assert(kUnpackThreads == 256, "the column-sum reduction assumes 256 unpack threads (32 rows x 8 chunks per pass)");
+    static_assert(kRowsPerStage >= 1 && kRowsPerStage <= 16 && 16 % kRowsPerStage == 0, "stage size vs column-sum lanes");
 };
 
 constexpr int kWarpTma = 0;
@@ -69,6 +96,7 @@ struct KernelParams {
     const Segment *segments;       // device
     const int32_t *worker_begin;   // device, n_workers + 1
     int32_t *acc;                  // device accumulator slots, layout.hpp
+    int32_t *sums;                 // device column-sum slots, layout.hpp
     int first_frame;               // 1: first frame of an integration -> epilogue stores; 0: load-add-store
     int n_inputs;
     int n_freq;
@@ -76,24 +104,11 @@ struct KernelParams {
 };
 
 // ------------------------------------------------------------------------------------------------
-// a2: nibble unpack, 4 samples per 32-bit word.  Re = sext4(b >> 4), Im = sext4(b & 15)  (R2, R3)
+// a2: nibble unpack, 4 samples per 32-bit word, to OFFSET values x' = sext4(nibble) + 8 = nibble ^ 8  (R2, R3)
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t unpack_re4(uint32_t w)
-{
-    uint32_t sign;                                               // each byte -> 0xFF if its bit 7 is set else 0x00
-    asm("prmt.b32 %0, %1, %1, 0xBA98;" : "=r"(sign) : "r"(w));    // (selector bit 3 = replicate the byte's sign; __byte_perm masks it off)
-    return ((w >> 4) & 0x0F0F0F0Fu) | (sign & 0xF0F0F0F0u);
-}
-__device__ __forceinline__ uint32_t unpack_im4(uint32_t w)
-{
-    const uint32_t sign = (w & 0x08080808u) * 0x1Eu;             // 0x08 -> 0xF0 inside each byte, no carries
-    return (w & 0x0F0F0F0Fu) | sign;
-}
-// per-byte two's-complement negation of values in [-8, 7] (result in [-7, 8], fits int8)
-__device__ __forceinline__ uint32_t negate4(uint32_t y)
-{
-    return (0x80808080u - (y & 0x7F7F7F7Fu)) ^ (~y & 0x80808080u);
-}
+__device__ __forceinline__ uint32_t unpack_re4(uint32_t w) { return ((w >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u; }   // h' = Re + 8
+__device__ __forceinline__ uint32_t unpack_im4(uint32_t w) { return (w & 0x0F0F0F0Fu) ^ 0x08080808u; }          // l' = Im + 8
+__device__ __forceinline__ uint32_t complement4(uint32_t y) { return y ^ 0x0F0F0F0Fu; }                          // 15 - y per byte
 
 // ------------------------------------------------------------------------------------------------
 // the kernel
@@ -108,13 +123,19 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     const uint32_t warp = threadIdx.x >> 5;
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t rank = ptx::cluster_ctarank();          // 0 = leader (issues the MMAs)
+#ifdef XC_PROFILE
+    const long long prof_c0 = clock64();
+    unsigned long long prof_g0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(prof_g0));
+#endif
     const uint32_t worker = blockIdx.x >> 1;
 
     // ---- shared memory carve-up (1024-byte aligned data, then barriers) ----
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t smem_packed = smem_base;
     const uint32_t smem_planes = smem_packed + Cfg::kPackedStages * Cfg::kPackedStageBytes;
-    const uint32_t bar_base = smem_planes + Cfg::kPlaneStages * Cfg::kPlaneStageBytes;
+    const uint32_t smem_sumscratch = smem_planes + Cfg::kPlaneStages * Cfg::kPlaneStageBytes;
+    const uint32_t bar_base = smem_sumscratch + Cfg::kSumScratch;
     // barrier slots (8 bytes each)
     auto bar_pk_full = [&](int s) { return bar_base + 8u * (uint32_t)s; };
     auto bar_pk_empty = [&](int s) { return bar_base + 8u * (uint32_t)(Cfg::kPackedStages + s); };
@@ -157,6 +178,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         // ===================================================== a1: TMA producer (one lane)
         if (lane == 0) {
             uint32_t it = 0;
+            XC_PROF_DECL(w_pk_empty);
             for (int sg = seg_begin; sg < seg_end; ++sg) {
                 const Segment seg = p.segments[sg];
                 const int n_a = seg.I * kSuper + (int)rank * kBlock;
@@ -164,7 +186,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
                     const uint32_t slot = it % Cfg::kPackedStages;
                     const uint32_t ph = (it / Cfg::kPackedStages) & 1u;
+                    XC_PROF_BEGIN(w_pk_empty);
                     ptx::mbar_wait(bar_pk_empty(slot), ph ^ 1u);
+                    XC_PROF_END(w_pk_empty);
                     const uint32_t dst = smem_packed + slot * Cfg::kPackedStageBytes;
                     const bool off = kOffDiag && (seg.I != seg.J);
                     ptx::mbar_arrive_expect_tx(bar_pk_full(slot), off ? 2 * Cfg::kPlaneBytes : Cfg::kPlaneBytes);
@@ -172,6 +196,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                     if (off) ptx::tma_load_3d(dst + Cfg::kPlaneBytes, &frame_map, bar_pk_full(slot), n_b, seg.f, st * kStageT);
                 }
             }
+            XC_PROF_STORE(0, w_pk_empty);
         }
     } else if (warp == kWarpMma) {
         // ===================================================== a3: MMA issuer (leader CTA, one lane)
@@ -180,15 +205,23 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             const uint32_t tmem_R = tmem_base;
             const uint32_t tmem_Q = tmem_base + 256;
             uint32_t it = 0, unit = 0;
+            XC_PROF_DECL(w_acc_empty);
+            XC_PROF_DECL(w_pl_full);
+            XC_PROF_DECL(t_mma);
+            XC_PROF_BEGIN(t_mma);
             for (int sg = seg_begin; sg < seg_end; ++sg, ++unit) {
                 const Segment seg = p.segments[sg];
                 const bool off = kOffDiag && (seg.I != seg.J);
+                XC_PROF_BEGIN(w_acc_empty);
                 ptx::mbar_wait_cluster(bar_acc_empty, (unit & 1u) ^ 1u);     // epilogues of both CTAs drained TMEM
+                XC_PROF_END(w_acc_empty);
                 ptx::tc_fence_after_sync();
                 for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
                     const uint32_t slot = it % Cfg::kPlaneStages;
                     const uint32_t ph = (it / Cfg::kPlaneStages) & 1u;
+                    XC_PROF_BEGIN(w_pl_full);
                     ptx::mbar_wait_cluster(bar_pl_full(slot), ph);
+                    XC_PROF_END(w_pl_full);
                     ptx::tc_fence_after_sync();
                     const uint32_t pl = smem_planes + slot * Cfg::kPlaneStageBytes;
 #pragma unroll
@@ -215,52 +248,138 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 }
                 ptx::mma_commit<2>(bar_acc_full, 0x3);             // accumulators complete (both CTAs)
             }
+            XC_PROF_END(t_mma);
+            XC_PROF_STORE(1, w_acc_empty);
+            XC_PROF_STORE(2, w_pl_full);
+            XC_PROF_STORE(3, t_mma);
         }
     } else if (warp >= kWarpUnpack0 && warp < (uint32_t)Cfg::kWarpEpi0) {
         // ===================================================== a2: unpack warps
-        const uint32_t tid = threadIdx.x - kWarpUnpack0 * 32;     // 0 .. kUnpackThreads-1
+        // Thread `tid` handles the 16-byte chunk at byte offset (q * 256 + tid) * 16 of every 8 KiB block: row 32 q + tid / 8,
+        // chunk position tid % 8.  TMA's 128-byte swizzle puts logical chunk c of row k at position c ^ (k % 8), so the thread
+        // always sees the same 16 inputs  [16 c_t, 16 c_t + 16),  c_t = (tid % 8) ^ ((tid / 8) % 8)  -- which is what lets it
+        // keep their column sums in registers: byte lanes (<= 16 rows), widened to 16-bit lanes (<= 4096 rows), reduced over
+        // the 32 threads that share a chunk through smem into an int32 total held by thread `input index` (< 128).
+        const uint32_t tid = threadIdx.x - kWarpUnpack0 * 32;     // 0 .. 255
         const uint32_t pl_full_leader = ptx::mapa(bar_base, 0) + (bar_pl_full(0) - bar_base);
+        uint32_t bsum[Cfg::kSumPlanes][4];    // byte lanes   : word k = inputs 4k .. 4k+3 of the chunk
+        uint32_t wsum[Cfg::kSumPlanes][8];    // 16-bit lanes : [k] = bytes 0, 2 of word k ; [4 + k] = bytes 1, 3
+        uint32_t tot[Cfg::kSumPlanes];        // tid < 128: int32 column sum of input `tid` of the block, this segment so far
+#pragma unroll
+        for (int pl = 0; pl < Cfg::kSumPlanes; ++pl) {
+            tot[pl] = 0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) bsum[pl][k] = 0;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) wsum[pl][k] = 0;
+        }
+        auto widen = [&]() {
+#pragma unroll
+            for (int pl = 0; pl < Cfg::kSumPlanes; ++pl)
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    wsum[pl][k] += bsum[pl][k] & 0x00FF00FFu;
+                    wsum[pl][4 + k] += (bsum[pl][k] >> 8) & 0x00FF00FFu;
+                    bsum[pl][k] = 0;
+                }
+        };
+        // where thread `tid` (< 128, input index inside the block) finds its input in a contributor's 32-byte record
+        const uint32_t red_chunk = tid >> 4;
+        const uint32_t red_off = ((((tid & 1u) << 2) + ((tid & 15u) >> 2)) << 2) + (((tid & 3u) >> 1) << 1);
+        auto flush = [&](int n_planes) {
+            widen();
+#pragma unroll
+            for (int pl = 0; pl < Cfg::kSumPlanes; ++pl) {
+                if (pl < n_planes) {
+                    const uint32_t rec = smem_sumscratch + tid * 32u;
+                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rec), "r"(wsum[pl][0]), "r"(wsum[pl][1]), "r"(wsum[pl][2]),
+                                 "r"(wsum[pl][3])
+                                 : "memory");
+                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rec + 16u), "r"(wsum[pl][4]), "r"(wsum[pl][5]),
+                                 "r"(wsum[pl][6]), "r"(wsum[pl][7])
+                                 : "memory");
+                    asm volatile("bar.sync 1, 256;" ::: "memory");
+                    if (tid < 128) {
+                        uint32_t acc = 0;
+#pragma unroll 8
+                        for (uint32_t row = 0; row < 32; ++row) {
+                            const uint32_t contributor = 8u * row + (red_chunk ^ (row & 7u));
+                            uint32_t v;
+                            asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(smem_sumscratch + contributor * 32u + red_off));
+                            acc += v;
+                        }
+                        tot[pl] += acc;
+                    }
+                    asm volatile("bar.sync 1, 256;" ::: "memory");
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) wsum[pl][k] = 0;
+                }
+            }
+        };
         uint32_t it = 0;
+        XC_PROF_DECL(w_pk_full);
+        XC_PROF_DECL(w_pl_empty);
+        XC_PROF_DECL(t_flush);
+        XC_PROF_DECL(t_unpack);
+        XC_PROF_BEGIN(t_unpack);
         for (int sg = seg_begin; sg < seg_end; ++sg) {
             const Segment seg = p.segments[sg];
             const bool off = kOffDiag && (seg.I != seg.J);
+            int since_widen = 0, since_flush = 0;
             for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
                 const uint32_t pslot = it % Cfg::kPackedStages, pph = (it / Cfg::kPackedStages) & 1u;
                 const uint32_t lslot = it % Cfg::kPlaneStages, lph = (it / Cfg::kPlaneStages) & 1u;
+                XC_PROF_BEGIN(w_pk_full);
                 ptx::mbar_wait(bar_pk_full(pslot), pph);                      // TMA bytes landed
+                XC_PROF_END(w_pk_full);
+                XC_PROF_BEGIN(w_pl_empty);
                 ptx::mbar_wait_cluster(bar_pl_empty(lslot), lph ^ 1u);        // MMAs that read this plane slot retired
+                XC_PROF_END(w_pl_empty);
                 const uint32_t src = smem_packed + pslot * Cfg::kPackedStageBytes;
                 const uint32_t dst = smem_planes + lslot * Cfg::kPlaneStageBytes;
 #pragma unroll
-                for (int q = 0; q < Cfg::kPlaneBytes / (Cfg::kUnpackThreads * 16); ++q) {
+                for (int q = 0; q < Cfg::kRowsPerStage; ++q) {
                     const uint32_t o = (uint32_t)(q * Cfg::kUnpackThreads + tid) * 16u;
-                    uint32_t w0, w1, w2, w3;
-                    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3) : "r"(src + o));
-                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + o), "r"(unpack_re4(w0)), "r"(unpack_re4(w1)),
-                                 "r"(unpack_re4(w2)), "r"(unpack_re4(w3))
-                                 : "memory");
-                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + Cfg::kPlaneBytes + o), "r"(unpack_im4(w0)),
-                                 "r"(unpack_im4(w1)), "r"(unpack_im4(w2)), "r"(unpack_im4(w3))
+                    uint32_t w[4], re[4], im[4];
+                    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(src + o));
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        re[k] = unpack_re4(w[k]);
+                        im[k] = unpack_im4(w[k]);
+                        bsum[0][k] += re[k];
+                        bsum[1][k] += im[k];
+                    }
+                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + o), "r"(re[0]), "r"(re[1]), "r"(re[2]), "r"(re[3]) : "memory");
+                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + Cfg::kPlaneBytes + o), "r"(im[0]), "r"(im[1]), "r"(im[2]),
+                                 "r"(im[3])
                                  : "memory");
                 }
-                if (off) {
+                if constexpr (kOffDiag) {
+                    if (off) {
 #pragma unroll
-                    for (int q = 0; q < Cfg::kPlaneBytes / (Cfg::kUnpackThreads * 16); ++q) {
-                        const uint32_t o = (uint32_t)(q * Cfg::kUnpackThreads + tid) * 16u;
-                        uint32_t w0, w1, w2, w3;
-                        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                                     : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3)
-                                     : "r"(src + Cfg::kPlaneBytes + o));
-                        const uint32_t i0 = unpack_im4(w0), i1 = unpack_im4(w1), i2 = unpack_im4(w2), i3 = unpack_im4(w3);
-                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 2 * Cfg::kPlaneBytes + o), "r"(unpack_re4(w0)),
-                                     "r"(unpack_re4(w1)), "r"(unpack_re4(w2)), "r"(unpack_re4(w3))
-                                     : "memory");
-                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 3 * Cfg::kPlaneBytes + o), "r"(i0), "r"(i1), "r"(i2),
-                                     "r"(i3)
-                                     : "memory");
-                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 4 * Cfg::kPlaneBytes + o), "r"(negate4(i0)),
-                                     "r"(negate4(i1)), "r"(negate4(i2)), "r"(negate4(i3))
-                                     : "memory");
+                        for (int q = 0; q < Cfg::kRowsPerStage; ++q) {
+                            const uint32_t o = (uint32_t)(q * Cfg::kUnpackThreads + tid) * 16u;
+                            uint32_t w[4], re[4], im[4];
+                            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                         : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3])
+                                         : "r"(src + Cfg::kPlaneBytes + o));
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                re[k] = unpack_re4(w[k]);
+                                im[k] = unpack_im4(w[k]);
+                                bsum[Cfg::kSumPlanes - 2][k] += re[k];
+                                bsum[Cfg::kSumPlanes - 1][k] += im[k];
+                            }
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 2 * Cfg::kPlaneBytes + o), "r"(re[0]), "r"(re[1]),
+                                         "r"(re[2]), "r"(re[3])
+                                         : "memory");
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 3 * Cfg::kPlaneBytes + o), "r"(im[0]), "r"(im[1]),
+                                         "r"(im[2]), "r"(im[3])
+                                         : "memory");
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 4 * Cfg::kPlaneBytes + o), "r"(complement4(im[0])),
+                                         "r"(complement4(im[1])), "r"(complement4(im[2])), "r"(complement4(im[3]))
+                                         : "memory");
+                        }
                     }
                 }
                 ptx::fence_proxy_async_smem();       // my plane writes -> visible to the tensor core's smem reads
@@ -269,17 +388,43 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                     ptx::mbar_arrive_local(bar_pk_empty(pslot));                       // packed slot may be refilled
                     ptx::mbar_arrive_cluster(pl_full_leader + 8u * lslot);             // tell the leader's MMA thread
                 }
+                if (++since_widen == Cfg::kWidenStages) { widen(); since_widen = 0; }
+                if (++since_flush == Cfg::kFlushStages) { flush(off ? 4 : 2); since_flush = 0; since_widen = 0; }
             }
+            // segment done: this segment's column sums -> its sum slot (same store / load-add-store rule as the epilogue)
+            XC_PROF_BEGIN(t_flush);
+            flush(off ? 4 : 2);
+            XC_PROF_END(t_flush);
+            if (tid < 128) {
+                int32_t *dst_sum = p.sums + ((size_t)seg.slot * 2 + rank) * (size_t)kSumElemsPerCta + tid;
+#pragma unroll
+                for (int pl = 0; pl < Cfg::kSumPlanes; ++pl) {
+                    if (pl < (off ? 4 : 2)) {
+                        const int32_t old = p.first_frame ? 0 : dst_sum[pl * kBlock];
+                        dst_sum[pl * kBlock] = old + (int32_t)tot[pl];
+                    }
+                    tot[pl] = 0;
+                }
+            }
+        }
+        XC_PROF_END(t_unpack);
+        if (tid == 0) {
+            XC_PROF_STORE(4, w_pk_full);
+            XC_PROF_STORE(5, w_pl_empty);
+            XC_PROF_STORE(6, t_flush);
+            XC_PROF_STORE(7, t_unpack);
         }
     } else if (warp >= (uint32_t)Cfg::kWarpEpi0) {
         // ===================================================== a4: epilogue warps
         const uint32_t quarter = warp & 3u;                      // TMEM lanes [32*quarter, 32*quarter+32)
         const uint32_t acc_empty_leader = ptx::mapa(bar_acc_empty, 0);
         uint32_t unit = 0;
+        XC_PROF_DECL(t_epi);
         for (int sg = seg_begin; sg < seg_end; ++sg, ++unit) {
             const Segment seg = p.segments[sg];
             ptx::mbar_wait_cluster(bar_acc_full, unit & 1u);
             ptx::tc_fence_after_sync();
+            XC_PROF_BEGIN(t_epi);
             const int row0 = (int)(rank * kBlock + quarter * 32);             // first row of this warp inside the super-block
             const int rows_valid = p.n_inputs - seg.I * kSuper - row0;         // rows of this warp that are real inputs
             const int cols_valid = min(kSuper, p.n_inputs - seg.J * kSuper);   // columns that are real inputs
@@ -319,7 +464,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             ptx::tc_fence_before_sync();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive_cluster(acc_empty_leader);          // TMEM may be overwritten by the next unit
+            XC_PROF_END(t_epi);
         }
+        if (warp == (uint32_t)Cfg::kWarpEpi0 && lane == 0) XC_PROF_STORE(8, t_epi);
     }
 
     // ---- teardown: everyone in both CTAs done with TMEM / peer smem before dealloc and exit ----
@@ -330,6 +477,16 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         ptx::tc_fence_after_sync();
         ptx::tmem_dealloc<2>(tmem_base, kAccCols);
     }
+#ifdef XC_PROFILE
+    if (threadIdx.x == 0) {
+        unsigned long long prof_g1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(prof_g1));
+        g_prof[blockIdx.x][9] = (unsigned long long)(clock64() - prof_c0);
+        g_prof[blockIdx.x][10] = prof_g1 - prof_g0;
+        g_prof[blockIdx.x][11] = prof_g0;
+        g_prof[blockIdx.x][12] = prof_g1;
+    }
+#endif
 }
 
 }  // namespace xc

@@ -147,6 +147,24 @@ def test_int32_stays_exact_at_the_bound(xb):
     x.close()
 
 
+def test_offset_operands_wrap_modulo_2_32(xb):
+    # The tensor core is fed x + 8; the offset sums R', Q' reach 450 * T and wrap modulo 2^32 long before
+    # the true visibilities (|V| <= 128 * T) leave int32.  xcorr_read's offset removal must still be exact.
+    t = 16_777_215
+    x = xb.XCorr(16, 1, t)
+    fr = torch.empty((t, 16), dtype=torch.uint8, device="cuda")
+    fr[:, 0::2] = 0x77        #  7 + 7i  -> offset operands 15, 15 (largest products)
+    fr[:, 1::2] = 0x87        # -8 + 7i
+    x.process(fr.reshape(-1))
+    got = x.read().cpu().numpy()[0].astype(np.int64)
+    x.close()
+    vals = {0: 7 + 7j, 1: -8 + 7j}
+    for i in range(16):
+        for j in range(i, 16):
+            v = vals[i % 2] * np.conj(vals[j % 2]) * t
+            assert got[oracle.pair_index(16, i, j)].tolist() == [int(v.real), int(v.imag)], (i, j)
+
+
 # ------------------------------------------------------------------ streamed path (a5)
 def test_streamed_path_matches_oracle(xb):
     n, f, t = 256, 4, 256
