@@ -377,3 +377,11 @@ extern "C" int xcorr_debug_process_simt(xcorr_handle *h, const void *packed_fram
     h->clean = false;
     return XCORR_OK;
 }
+
+#ifdef XC_PROFILE
+// development builds only (-DXC_PROFILE): per-CTA stall counters of the last xengine_kernel launch, [1024][16] uint64
+extern "C" int xcorr_debug_read_profile(unsigned long long *out)
+{
+    return cudaMemcpyFromSymbol(out, g_prof, sizeof(unsigned long long) * 1024 * 16) == cudaSuccess ? XCORR_OK : XCORR_ECUDA;
+}
+#endif

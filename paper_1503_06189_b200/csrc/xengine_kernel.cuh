@@ -223,6 +223,14 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                     ptx::mbar_wait_cluster(bar_pl_full(slot), ph);
                     XC_PROF_END(w_pl_full);
                     ptx::tc_fence_after_sync();
+#ifdef XC_PROFILE
+                    if (it == 0) {
+                        unsigned long long g;
+                        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
+                        g_prof[blockIdx.x][13] = (unsigned long long)(clock64() - prof_c0);
+                        g_prof[blockIdx.x][14] = g - prof_g0;
+                    }
+#endif
                     const uint32_t pl = smem_planes + slot * Cfg::kPlaneStageBytes;
 #pragma unroll
                     for (int k = 0; k < kStageT / 32; ++k) {
@@ -231,9 +239,24 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                         const uint64_t d_la = ptx::make_smem_desc_mn_sw128(pl + 1 * Cfg::kPlaneBytes + koff, 1024, 1024);
                         const uint32_t acc = (st != seg.stage_begin || k != 0) ? 1u : 0u;
                         if (!off) {
+#ifdef XC_EXP_N128   // timing experiment only (wrong results): same tensor work as N = 128 halves, A read twice
+                            constexpr uint32_t idesc_h = ptx::make_idesc_i8_mnmajor(256, 128);
+                            ptx::mma_i8<2>(tmem_R, d_ha, d_ha, idesc_h, acc);
+                            ptx::mma_i8<2>(tmem_R + 128, d_ha, d_ha, idesc_h, acc);
+                            ptx::mma_i8<2>(tmem_R, d_la, d_la, idesc_h, 1u);
+                            ptx::mma_i8<2>(tmem_R + 128, d_la, d_la, idesc_h, 1u);
+                            ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc_h, acc);
+                            ptx::mma_i8<2>(tmem_Q + 128, d_la, d_ha, idesc_h, acc);
+#elif defined(XC_EXP_2P5)   // timing experiment only (wrong results): 2.5 MMAs per K-step
+                            constexpr uint32_t idesc_h = ptx::make_idesc_i8_mnmajor(256, 128);
+                            ptx::mma_i8<2>(tmem_R, d_ha, d_ha, idesc, acc);
+                            ptx::mma_i8<2>(tmem_R, d_la, d_la, idesc_h, 1u);
+                            ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc, acc);
+#else
                             ptx::mma_i8<2>(tmem_R, d_ha, d_ha, idesc, acc);   // R  = h h^T
                             ptx::mma_i8<2>(tmem_R, d_la, d_la, idesc, 1u);    // R += l l^T
                             ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc, acc);   // Q  = l h^T
+#endif
                         } else {
                             const uint64_t d_hb = ptx::make_smem_desc_mn_sw128(pl + 2 * Cfg::kPlaneBytes + koff, 1024, 1024);
                             const uint64_t d_lb = ptx::make_smem_desc_mn_sw128(pl + 3 * Cfg::kPlaneBytes + koff, 1024, 1024);
@@ -249,6 +272,13 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 ptx::mma_commit<2>(bar_acc_full, 0x3);             // accumulators complete (both CTAs)
             }
             XC_PROF_END(t_mma);
+#ifdef XC_PROFILE
+            {
+                unsigned long long g;
+                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
+                g_prof[blockIdx.x][15] = g - prof_g0;
+            }
+#endif
             XC_PROF_STORE(1, w_acc_empty);
             XC_PROF_STORE(2, w_pl_full);
             XC_PROF_STORE(3, t_mma);
