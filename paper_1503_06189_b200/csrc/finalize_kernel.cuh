@@ -40,7 +40,10 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
                                                         uint32_t offset_samples)
 {
     const int bj = blockIdx.x, bi = blockIdx.y, f = blockIdx.z;
+    // PDL (griddepcontrol): let the next kernel of the stream start its prologue; wait for the producer of the slots
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (bj < bi) return;
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     __shared__ uint32_t sR[32][33];   // [col][row]
     __shared__ uint32_t sQ[32][33];   // [col][row]
     __shared__ uint32_t sX[32][33];   // [row j][col i] of the transposed patch (diagonal super-tiles only)

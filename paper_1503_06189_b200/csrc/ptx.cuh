@@ -28,6 +28,12 @@ __device__ __forceinline__ uint32_t mapa(uint32_t local, uint32_t rank)
     return r;
 }
 
+// ---------------------------------------------------------------- programmatic dependent launch (PDL)
+// launch_dependents: the next kernel in the stream (if launched with programmatic stream serialization) may start
+// its prologue now.  wait: block until every prerequisite grid has completed and its memory is visible.
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // ---------------------------------------------------------------- mbarrier
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {

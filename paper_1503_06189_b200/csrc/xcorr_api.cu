@@ -178,7 +178,11 @@ static int encode_frame_map(xcorr_handle *h, const void *frame_dev, CUtensorMap 
     // a1: global uint8[T][F][N] seen as a 3-D tensor (n, f, t); one box = 128 inputs x 1 channel x kStageT samples,
     // written to smem as kStageT rows of 128 bytes with the 128-byte swizzle the MMA descriptors expect.
     const cuuint64_t dims[3] = {(cuuint64_t)h->n_inputs, (cuuint64_t)h->n_freq, (cuuint64_t)h->n_time};
+#ifdef XC_EXP_FMAJOR   // timing experiment only (wrong results): frame read as [f][t][n], i.e. contiguous boxes
+    const cuuint64_t strides[2] = {(cuuint64_t)h->n_inputs * (cuuint64_t)h->n_time, (cuuint64_t)h->n_inputs};
+#else
     const cuuint64_t strides[2] = {(cuuint64_t)h->n_inputs, (cuuint64_t)h->n_inputs * (cuuint64_t)h->n_freq};
+#endif
     const cuuint32_t box[3] = {(cuuint32_t)kBlock, 1u, (cuuint32_t)kStageT};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void *>(frame_dev), dims, strides, box, estr,
@@ -217,11 +221,25 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
     p.n_freq = h->n_freq;
     p.n_time = h->n_time;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    const dim3 grid(2 * h->n_workers);
-    if (h->offdiag)
-        xengine_kernel<true><<<grid, KernelCfg<true>::kThreads, KernelCfg<true>::kSmemBytes, s>>>(map, p);
-    else
-        xengine_kernel<false><<<grid, KernelCfg<false>::kThreads, KernelCfg<false>::kSmemBytes, s>>>(map, p);
+    // programmatic dependent launch: this kernel's prologue (barrier init, TMEM allocation, cluster sync) may overlap the
+    // tail of the previous kernel of the stream; the kernel itself waits (griddepcontrol.wait) before touching memory
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2 * h->n_workers);
+    cfg.stream = s;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (h->offdiag) {
+        cfg.blockDim = dim3(KernelCfg<true>::kThreads);
+        cfg.dynamicSmemBytes = KernelCfg<true>::kSmemBytes;
+        XC_CUDA(h, cudaLaunchKernelEx(&cfg, xengine_kernel<true>, map, p));
+    } else {
+        cfg.blockDim = dim3(KernelCfg<false>::kThreads);
+        cfg.dynamicSmemBytes = KernelCfg<false>::kSmemBytes;
+        XC_CUDA(h, cudaLaunchKernelEx(&cfg, xengine_kernel<false>, map, p));
+    }
     XC_CUDA(h, cudaGetLastError());
     h->launches += 1;
     h->samples_since_read += h->n_time;
@@ -247,8 +265,19 @@ extern "C" int xcorr_read(xcorr_handle *h, int32_t *upper_triangle_out, void *cu
         XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, s));
         XC_CUDA(h, cudaMemsetAsync(h->sums, 0, h->sums_bytes, s));
     }
-    finalize_kernel<<<dim3(nt, nt, h->n_freq), 256, 0, s>>>(h->acc, h->sums, h->tile_slot_begin, dst, h->n_inputs,
-                                                            (uint32_t)h->offset_samples);
+    {
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(nt, nt, h->n_freq);
+        cfg.blockDim = dim3(256);
+        cfg.stream = s;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        XC_CUDA(h, cudaLaunchKernelEx(&cfg, finalize_kernel, (const int32_t *)h->acc, (const int32_t *)h->sums,
+                                      (const int32_t *)h->tile_slot_begin, dst, h->n_inputs, (uint32_t)h->offset_samples));
+    }
     XC_CUDA(h, cudaGetLastError());
     h->launches += 1;
     // ends the integration: no clearing pass -- the next frame's epilogue overwrites its slots (first_frame)

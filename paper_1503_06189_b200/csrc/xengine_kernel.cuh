@@ -145,11 +145,24 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     const uint32_t bar_acc_empty = bar_acc_full + 8u;
     const uint32_t tmem_slot = bar_acc_empty + 8u;   // uint32 written by tcgen05.alloc
 
+    // PDL: the next kernel of the stream may begin its own prologue; it waits (grid_dependency_wait) for this grid's completion
+    ptx::grid_launch_dependents();
+
+    const int seg_begin = p.worker_begin[worker];          // static schedule tables: not written by any kernel
+    const int seg_end = p.worker_begin[worker + 1];
+
+    // a1 issues one packed stage: one box (two when I < J) of kStageT rows x 128 inputs, 128-byte swizzle
+    auto tma_issue = [&](const Segment &seg, int st, uint32_t slot) {
+        const uint32_t dst = smem_packed + slot * Cfg::kPackedStageBytes;
+        const bool off = kOffDiag && (seg.I != seg.J);
+        ptx::mbar_arrive_expect_tx(bar_pk_full(slot), off ? 2 * Cfg::kPlaneBytes : Cfg::kPlaneBytes);
+        ptx::tma_load_3d(dst, &frame_map, bar_pk_full(slot), seg.I * kSuper + (int)rank * kBlock, seg.f, st * kStageT);
+        if (off)
+            ptx::tma_load_3d(dst + Cfg::kPlaneBytes, &frame_map, bar_pk_full(slot), seg.J * kSuper + (int)rank * kBlock, seg.f, st * kStageT);
+    };
+    uint32_t tma_pre = 0;   // packed stages the TMA lane put in flight before the prologue barrier (their slots start empty)
+
     if (warp == kWarpMma && lane == 0) {
-        for (int s = 0; s < Cfg::kPackedStages; ++s) {
-            ptx::mbar_init(bar_pk_full(s), 1);                    // TMA producer's arrive.expect_tx
-            ptx::mbar_init(bar_pk_empty(s), Cfg::kUnpackWarps);     // one arrive per unpack warp
-        }
         for (int s = 0; s < Cfg::kPlaneStages; ++s) {
             ptx::mbar_init(bar_pl_full(s), 2 * Cfg::kUnpackWarps);  // unpack warps of BOTH CTAs (used in the leader only)
             ptx::mbar_init(bar_pl_empty(s), 1);                   // tcgen05.commit (multicast to both CTAs)
@@ -158,7 +171,23 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         ptx::mbar_init(bar_acc_empty, 2 * kNumEpiWarps);          // epilogue warps of BOTH CTAs (leader only)
         ptx::fence_mbar_init();
     }
-    if (warp == kWarpTma && lane == 0) ptx::prefetch_tensormap(&frame_map);
+    if (warp == kWarpTma && lane == 0) {
+        ptx::prefetch_tensormap(&frame_map);
+        for (int s = 0; s < Cfg::kPackedStages; ++s) {
+            ptx::mbar_init(bar_pk_full(s), 1);                    // TMA producer's arrive.expect_tx
+            ptx::mbar_init(bar_pk_empty(s), Cfg::kUnpackWarps);     // one arrive per unpack warp
+        }
+        ptx::fence_mbar_init();
+        ptx::fence_proxy_async_smem();
+        // the packed barriers and slots are this CTA's own: start the first loads now, so the frame is already on its
+        // way while TMEM is allocated and the cluster synchronises
+        ptx::grid_dependency_wait();                              // the frame may be the previous kernel's output
+        for (int sg = seg_begin; sg < seg_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++sg) {
+            const Segment seg = p.segments[sg];
+            for (int st = seg.stage_begin; st < seg.stage_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++st, ++tma_pre)
+                tma_issue(seg, st, tma_pre);
+        }
+    }
     if (warp == kWarpTmem) {
         ptx::tmem_alloc<2>(tmem_slot, kAccCols);
         ptx::tmem_relinquish<2>();
@@ -167,12 +196,10 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     __syncthreads();
     ptx::cluster_sync();           // barriers of both CTAs initialised before any remote arrive / multicast commit
     ptx::tc_fence_after_sync();
+    ptx::grid_dependency_wait();   // accumulator / sum slots: the previous kernel of the stream may still read or write them
 
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
-
-    const int seg_begin = p.worker_begin[worker];
-    const int seg_end = p.worker_begin[worker + 1];
 
     if (warp == kWarpTma) {
         // ===================================================== a1: TMA producer (one lane)
@@ -181,19 +208,14 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             XC_PROF_DECL(w_pk_empty);
             for (int sg = seg_begin; sg < seg_end; ++sg) {
                 const Segment seg = p.segments[sg];
-                const int n_a = seg.I * kSuper + (int)rank * kBlock;
-                const int n_b = seg.J * kSuper + (int)rank * kBlock;
                 for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
+                    if (it < tma_pre) continue;                    // already in flight (prologue)
                     const uint32_t slot = it % Cfg::kPackedStages;
                     const uint32_t ph = (it / Cfg::kPackedStages) & 1u;
                     XC_PROF_BEGIN(w_pk_empty);
                     ptx::mbar_wait(bar_pk_empty(slot), ph ^ 1u);
                     XC_PROF_END(w_pk_empty);
-                    const uint32_t dst = smem_packed + slot * Cfg::kPackedStageBytes;
-                    const bool off = kOffDiag && (seg.I != seg.J);
-                    ptx::mbar_arrive_expect_tx(bar_pk_full(slot), off ? 2 * Cfg::kPlaneBytes : Cfg::kPlaneBytes);
-                    ptx::tma_load_3d(dst, &frame_map, bar_pk_full(slot), n_a, seg.f, st * kStageT);
-                    if (off) ptx::tma_load_3d(dst + Cfg::kPlaneBytes, &frame_map, bar_pk_full(slot), n_b, seg.f, st * kStageT);
+                    tma_issue(seg, st, slot);
                 }
             }
             XC_PROF_STORE(0, w_pk_empty);
@@ -239,7 +261,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                         const uint64_t d_la = ptx::make_smem_desc_mn_sw128(pl + 1 * Cfg::kPlaneBytes + koff, 1024, 1024);
                         const uint32_t acc = (st != seg.stage_begin || k != 0) ? 1u : 0u;
                         if (!off) {
-#ifdef XC_EXP_N128   // timing experiment only (wrong results): same tensor work as N = 128 halves, A read twice
+#ifdef XC_EXP_NOMMA   // power experiment only (wrong results): no MMAs issued
+                            (void)acc; (void)d_ha; (void)d_la;
+#elif defined(XC_EXP_N128)   // timing experiment only (wrong results): same tensor work as N = 128 halves, A read twice
                             constexpr uint32_t idesc_h = ptx::make_idesc_i8_mnmajor(256, 128);
                             ptx::mma_i8<2>(tmem_R, d_ha, d_ha, idesc_h, acc);
                             ptx::mma_i8<2>(tmem_R + 128, d_ha, d_ha, idesc_h, acc);
@@ -367,6 +391,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 XC_PROF_END(w_pl_empty);
                 const uint32_t src = smem_packed + pslot * Cfg::kPackedStageBytes;
                 const uint32_t dst = smem_planes + lslot * Cfg::kPlaneStageBytes;
+#ifdef XC_EXP_NOUNPACK   // power experiment only (wrong results): planes are never written
+                if (false)
+#endif
 #pragma unroll
                 for (int q = 0; q < Cfg::kRowsPerStage; ++q) {
                     const uint32_t o = (uint32_t)(q * Cfg::kUnpackThreads + tid) * 16u;
@@ -460,6 +487,14 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             const int cols_valid = min(kSuper, p.n_inputs - seg.J * kSuper);   // columns that are real inputs
             // this segment's own slot: [r][col/4][row][4] int32 -> one warp's 16-byte accesses are 512 B contiguous
             int32_t *slot_cta = p.acc + ((size_t)seg.slot * 2 + rank) * (size_t)kAccElemsPerCta + (size_t)(quarter * 32 + lane) * 4;
+            // this warp's last TMEM load has landed: the next unit's MMAs may overwrite the accumulators
+            bool released = false;
+            auto release_tmem = [&]() {
+                ptx::tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive_cluster(acc_empty_leader);
+                released = true;
+            };
 #ifdef XC_DEBUG_SKIP_EPI
             if (false) {
 #else
@@ -467,14 +502,14 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
 #endif
                 // R columns: on a diagonal super-tile only j >= i is ever read -> start at this warp's first row
                 const int r_begin = (seg.I == seg.J) ? row0 : 0;
-                const int n_chunks_r = (cols_valid - r_begin + 31) / 32;      // may be <= 0
-                const int n_chunks_q = (cols_valid + 31) / 32;
-                for (int ch = 0; ch < max(n_chunks_r, 0) + n_chunks_q; ++ch) {
-                    const int col = (ch < n_chunks_r) ? (r_begin + 32 * ch) : (256 + 32 * (ch - max(n_chunks_r, 0)));
-                    uint32_t v[32];
-                    ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + (uint32_t)col, v);
-                    ptx::tmem_wait_ld();
-                    int32_t *dst = slot_cta + (size_t)(col >> 2) * (kBlock * 4);
+                const int n_chunks_r = max((cols_valid - r_begin + 31) / 32, 0);
+                const int n_chunks = n_chunks_r + (cols_valid + 31) / 32;       // R chunks, then Q chunks (32 columns each)
+                auto chunk_col = [&](int ch) { return (ch < n_chunks_r) ? (r_begin + 32 * ch) : (256 + 32 * (ch - n_chunks_r)); };
+                auto chunk_load = [&](int ch, uint32_t (&v)[32]) {
+                    ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + (uint32_t)chunk_col(ch), v);
+                };
+                auto chunk_store = [&](int ch, const uint32_t (&v)[32]) {
+                    int32_t *dst = slot_cta + (size_t)(chunk_col(ch) >> 2) * (kBlock * 4);
                     if (p.first_frame) {
 #pragma unroll
                         for (int g = 0; g < 8; ++g)
@@ -489,11 +524,22 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                             ptx::st_global_v4(dst + g * (kBlock * 4), old[g].x + (int32_t)v[4 * g], old[g].y + (int32_t)v[4 * g + 1],
                                               old[g].z + (int32_t)v[4 * g + 2], old[g].w + (int32_t)v[4 * g + 3]);
                     }
+                };
+                // two register buffers: the TMEM load of chunk k+1 is in flight while chunk k is written out
+                uint32_t va[32], vb[32];
+                if (n_chunks > 0) chunk_load(0, va);
+                for (int ch = 0; ch < n_chunks; ch += 2) {
+                    ptx::tmem_wait_ld();
+                    if (ch + 1 < n_chunks) chunk_load(ch + 1, vb); else release_tmem();
+                    chunk_store(ch, va);
+                    if (ch + 1 < n_chunks) {
+                        ptx::tmem_wait_ld();
+                        if (ch + 2 < n_chunks) chunk_load(ch + 2, va); else release_tmem();
+                        chunk_store(ch + 1, vb);
+                    }
                 }
             }
-            ptx::tc_fence_before_sync();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive_cluster(acc_empty_leader);          // TMEM may be overwritten by the next unit
+            if (!released) release_tmem();
             XC_PROF_END(t_epi);
         }
         if (warp == (uint32_t)Cfg::kWarpEpi0 && lane == 0) XC_PROF_STORE(8, t_epi);
