@@ -137,3 +137,52 @@ CONFIGS = {
     "C4": Config("C4", 2048, 16, 8192, "gaussian_sky", 4, note="larger-N scaling, common sky signal"),
     "C5": Config("C5", 512, 32, 131072, "stress", 5, note="saturation / overflow stress, 2 GiB"),
 }
+
+
+# ----------------------------------------------------------------------------------------------------------
+# F-engine flags and packet loss (NEXT-1; NEXT-2).  Only draws and packs: the
+# normalisation arithmetic lives in the CUDA path and, separately, in oracle/normalisation.py.
+# ----------------------------------------------------------------------------------------------------------
+PACKET_T = 4      # time samples per UDP packet
+PACKET_F = 8      # frequency channels per 10 GbE stream / packet
+
+
+def pack_flags(flags: np.ndarray) -> np.ndarray:
+    """bool[T][F][N] -> wire bit-field uint8[T][F][N/8]: input n is bit (n % 8) of byte n // 8 (DESIGN.md N1)."""
+    flags = np.asarray(flags, dtype=bool)
+    if flags.shape[-1] % 8:
+        raise ValueError("N must be a multiple of 8")
+    return np.packbits(flags, axis=-1, bitorder="little")
+
+
+def draw_flags_and_loss(n_inputs: int, n_freq: int, n_time: int, seed: int, p_flag: float = 1e-3, p_burst: float = 2e-4,
+                        burst_frac: float = 0.05, p_packet_loss: float = 2e-3):
+    """Seeded F-engine flags and packet loss for one frame.
+
+    * each (t, f, n) sample is flagged independently with probability p_flag (ADC / FFT range errors);
+    * with probability p_burst a whole (t, f) sample has a further burst_frac of its inputs flagged at once
+      (several inputs flagged in the same time sample: the paper's intersections, PAPER.md:117);
+    * packets of PACKET_T samples x PACKET_F channels x all inputs are lost with probability p_packet_loss; a lost
+      packet carries no flags (its footer never arrived).
+    Returns flags bool[T][F][N], lost_mask bool[T][F], lost int32[F] (lost time samples per channel).
+    The paper gives no rates ("provided E << N"); these are this build's.
+    """
+    rng = np.random.default_rng(seed)
+    flags = rng.random((n_time, n_freq, n_inputs), dtype=np.float32) < np.float32(p_flag)
+    burst = rng.random((n_time, n_freq)) < p_burst
+    for t, f in zip(*np.nonzero(burst)):
+        flags[t, f] |= rng.random(n_inputs) < burst_frac
+    npt, npf = -(-n_time // PACKET_T), -(-n_freq // PACKET_F)
+    lost_pkt = rng.random((npt, npf)) < p_packet_loss
+    lost_mask = np.repeat(np.repeat(lost_pkt, PACKET_T, axis=0), PACKET_F, axis=1)[:n_time, :n_freq]
+    flags &= ~lost_mask[:, :, None]
+    lost = lost_mask.sum(axis=0).astype(np.int32)
+    return flags, lost_mask, lost
+
+
+def zero_lost_samples(frame: np.ndarray, flags: np.ndarray, lost_mask: np.ndarray) -> np.ndarray:
+    """"When this happens the data points are zeroed, before they are transferred to the GPU" (PAPER.md:113)."""
+    out = frame.copy()
+    out[flags] = 0
+    out[lost_mask] = 0
+    return out
