@@ -101,6 +101,55 @@ int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void *cuda_stre
  */
 int xcorr_read(xcorr_handle *h, int32_t *upper_triangle_out, void *cuda_stream);
 
+/* ---------------------------------------------------------------------------------------------------
+ * Lost-sample normalisation (SURVEY.md 8(f) NEXT-1; section II-C, :111-121).  Samples lost to packet
+ * loss or flagged by the F-engine are ZERO in the frame ("the data points are zeroed, before they are
+ * transferred to the GPU", :113), so some visibilities hold fewer samples.  The paper's post-processing builds a
+ * normalisation matrix -- a packet-loss counter added to every point (:115), per-(input, frequency) flag
+ * counters (:116), minus the per-sample intersections of inputs flagged together (:117-119) -- and applies the
+ * lost fraction to the correlation matrix (:121).  Readings N1..N5 in DESIGN.md section 12.
+ * ------------------------------------------------------------------------------------------------- */
+
+/*
+ * xcorr_norm_enable -- startup-time call (no allocation after startup): allocates the device
+ * flag-intersection accumulator int32[F][P] (zeroed), the packet-loss counters and the staging for host
+ * reads of the normalisation matrix.  Idempotent.  Must not be called in the middle of an integration.
+ * Errors: EINVAL, ENOMEM, ECUDA.
+ */
+int xcorr_norm_enable(xcorr_handle *h);
+
+/*
+ * xcorr_norm_process -- account for the lost samples of ONE frame (the frame given to xcorr_process before or
+ * after this call, in the same integration).  Either pointer may be NULL.
+ *
+ *   flags_dev          device pointer, F-engine flag bit-field of the frame, uint8[T][F][N/8]: input n of sample
+ *                      (t, f) is bit (n % 8) of byte n / 8; a set bit means that sample's voltage byte is zero in
+ *                      the frame.  16-byte aligned, BORROWED until `cuda_stream` has passed this call.  One launch
+ *                      of flag_count_kernel adds the per-sample intersections (and, on the diagonal, the flag
+ *                      counters) into the handle's accumulator.
+ *   lost_samples_host  HOST pointer, int32[F]: time samples of each channel lost with their packets in this
+ *                      frame (0 <= value <= T; the paper's packet-loss counter, kept per channel: a stream's
+ *                      counter applies to its 8 channels).  Read before the call returns.
+ * Errors: EINVAL (normalisation not enabled, misaligned, counter out of range), ECUDA.
+ */
+int xcorr_norm_process(xcorr_handle *h, const uint8_t *flags_dev, const int32_t *lost_samples_host, void *cuda_stream);
+
+/*
+ * xcorr_read_normalized -- xcorr_read() with the lost fraction applied, fused into the same kernel:
+ *
+ *   L[f][p(i,j)]  = lost[f] + c_f[i] + c_f[j] - #{samples with i and j both flagged}   (i != j)
+ *   L[f][p(i,i)]  = lost[f] + c_f[i]
+ *   vis_out       float32[F][P][2] = V * T / (T - L), T = samples integrated since the last read, computed in
+ *                 float32 (int32 -> float, one division, one multiplication, each rounded to nearest); 0 where
+ *                 T - L <= 0.  Pair order, host/device pointer rules and alignment as in xcorr_read.
+ *   lost_matrix_out  optional (NULL to skip): int32[F][P], the normalisation matrix L itself (exact).
+ *
+ * Ends the integration: visibilities, flag accumulator and loss counters start again from zero (a plain
+ * xcorr_read on a handle with normalisation enabled clears them as well).
+ * Errors: EINVAL, ECUDA.
+ */
+int xcorr_read_normalized(xcorr_handle *h, float *vis_out, int32_t *lost_matrix_out, void *cuda_stream);
+
 /* Release everything the handle owns (synchronises the device first).  NULL is a no-op. */
 void xcorr_destroy(xcorr_handle *h);
 

@@ -16,6 +16,7 @@ __all__ = [
     "XCORR_OK", "XCORR_EINVAL", "XCORR_EARCH", "XCORR_ENOMEM", "XCORR_ECUDA", "XCORR_EOVERFLOW",
     "XCorrError", "lib", "xcorr_create", "xcorr_process", "xcorr_read", "xcorr_destroy", "xcorr_strerror",
     "xcorr_last_cuda_error", "xcorr_frame_bytes", "xcorr_output_bytes", "xcorr_kernel_launches",
+    "xcorr_norm_enable", "xcorr_norm_process", "xcorr_read_normalized",
     "xcorr_stream_create", "xcorr_stream_submit", "xcorr_stream_sync", "xcorr_stream_read", "xcorr_stream_destroy",
     "xcorr_debug_schedule", "xcorr_debug_stage_samples", "xcorr_debug_process_simt", "XCorr", "XCorrStream",
 ]
@@ -67,6 +68,12 @@ def lib() -> ctypes.CDLL:
     L.xcorr_output_bytes.restype = ctypes.c_size_t
     L.xcorr_kernel_launches.argtypes = [vp]
     L.xcorr_kernel_launches.restype = ctypes.c_uint64
+    L.xcorr_norm_enable.argtypes = [vp]
+    L.xcorr_norm_enable.restype = ci
+    L.xcorr_norm_process.argtypes = [vp, vp, vp, vp]
+    L.xcorr_norm_process.restype = ci
+    L.xcorr_read_normalized.argtypes = [vp, vp, vp, vp]
+    L.xcorr_read_normalized.restype = ci
     L.xcorr_stream_create.argtypes = [vp, ci, ctypes.POINTER(vp)]
     L.xcorr_stream_create.restype = ci
     L.xcorr_stream_submit.argtypes = [vp, vp]
@@ -125,6 +132,18 @@ def xcorr_output_bytes(handle: int) -> int:
 
 def xcorr_kernel_launches(handle: int) -> int:
     return lib().xcorr_kernel_launches(handle)
+
+
+def xcorr_norm_enable(handle: int) -> int:
+    return lib().xcorr_norm_enable(handle)
+
+
+def xcorr_norm_process(handle: int, flags_dev: int, lost_samples_host: int, cuda_stream: int = 0) -> int:
+    return lib().xcorr_norm_process(handle, flags_dev or None, lost_samples_host or None, cuda_stream)
+
+
+def xcorr_read_normalized(handle: int, vis_out: int, lost_matrix_out: int = 0, cuda_stream: int = 0) -> int:
+    return lib().xcorr_read_normalized(handle, vis_out, lost_matrix_out or None, cuda_stream)
 
 
 def xcorr_stream_create(handle: int, depth: int = 2) -> tuple[int, int]:
@@ -226,6 +245,41 @@ class XCorr:
         if out.dtype != torch.int32 or not out.is_contiguous() or out.numel() * 4 != self.output_bytes:
             raise ValueError("out must be a contiguous int32 tensor of output_bytes bytes")
         self._check(xcorr_read(self.handle, out.data_ptr(), _stream_handle(stream)), "xcorr_read")
+        return out
+
+    # ---- lost-sample normalisation (NEXT-1)
+    def norm_enable(self) -> None:
+        self._check(xcorr_norm_enable(self.handle), "xcorr_norm_enable")
+
+    def norm_process(self, flags_dev=None, lost_samples=None, stream=None) -> None:
+        """flags_dev: CUDA uint8 tensor [T][F][N/8] or None; lost_samples: int32 numpy array [F] (host) or None."""
+        import numpy as np
+        fptr = 0
+        if flags_dev is not None:
+            if not flags_dev.is_cuda or not flags_dev.is_contiguous() or flags_dev.numel() * flags_dev.element_size() * 8 != self.frame_bytes:
+                raise ValueError("flags_dev must be a contiguous CUDA tensor of frame_bytes / 8 bytes")
+            fptr = flags_dev.data_ptr()
+        lptr = 0
+        if lost_samples is not None:
+            lost_samples = np.ascontiguousarray(lost_samples, dtype=np.int32)
+            if lost_samples.shape != (self.n_freq,):
+                raise ValueError("lost_samples must have shape (n_freq,)")
+            lptr = lost_samples.ctypes.data
+        self._check(xcorr_norm_process(self.handle, fptr, lptr, _stream_handle(stream)), "xcorr_norm_process")
+
+    def read_normalized(self, out=None, lost_out=None, stream=None):
+        """-> float32[F][P][2] (allocated on the device if None); lost_out: optional int32[F][P] tensor for L."""
+        import torch
+        if out is None:
+            out = torch.empty((self.n_freq, self.n_pairs, 2), dtype=torch.float32, device="cuda")
+        if out.dtype != torch.float32 or not out.is_contiguous() or out.numel() * 4 != self.output_bytes:
+            raise ValueError("out must be a contiguous float32 tensor of output_bytes bytes")
+        lptr = 0
+        if lost_out is not None:
+            if lost_out.dtype != torch.int32 or not lost_out.is_contiguous() or lost_out.numel() * 8 != self.output_bytes:
+                raise ValueError("lost_out must be a contiguous int32 tensor of n_freq * n_pairs elements")
+            lptr = lost_out.data_ptr()
+        self._check(xcorr_read_normalized(self.handle, out.data_ptr(), lptr, _stream_handle(stream)), "xcorr_read_normalized")
         return out
 
     def close(self) -> None:

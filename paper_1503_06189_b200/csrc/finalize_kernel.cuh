@@ -34,11 +34,22 @@ __device__ __forceinline__ uint4 slot_sum_v4(const int32_t *__restrict__ acc, in
     return s;
 }
 
-// grid (nt, nt, F), nt = ceil(N / 32); block 256 threads
+// Lost-sample normalisation fused into the write (normalise_kernel.cuh): inputs of the kNormalise variant
+struct NormParams {
+    const int32_t *x;        // device int32[F][P]: flag intersections, diagonal = flag counters
+    const int32_t *lost;     // device int32[F]: time samples lost with their packets, per channel
+    int32_t *lost_out;       // device int32[F][P] or nullptr: the normalisation matrix L itself
+    uint32_t n_samples;      // T: samples integrated since the last read
+};
+
+// grid (nt, nt, F), nt = ceil(N / 32); block 256 threads.  kNormalise = false: out = int32[F][P][2] (xcorr_read);
+// kNormalise = true: out = float32[F][P][2] = V * T / (T - L) (xcorr_read_normalized)
+template <bool kNormalise>
 __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict__ acc, const int32_t *__restrict__ sums,
-                                                        const int32_t *__restrict__ tile_slot_begin, int32_t *__restrict__ out, int n_inputs,
-                                                        uint32_t offset_samples)
+                                                        const int32_t *__restrict__ tile_slot_begin, void *__restrict__ out_v, int n_inputs,
+                                                        uint32_t offset_samples, const NormParams np)
 {
+    int32_t *__restrict__ out = reinterpret_cast<int32_t *>(out_v);
     const int bj = blockIdx.x, bi = blockIdx.y, f = blockIdx.z;
     // PDL (griddepcontrol): let the next kernel of the stream start its prologue; wait for the producer of the slots
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -86,6 +97,11 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
     // phase 2: tx <-> column j0 + tx, one output row per ty step: 8-byte (re, im) writes, 256 B contiguous per warp
     const long long P = (long long)n_inputs * (n_inputs + 1) / 2;
     const uint32_t shj = sS[2][tx], slj = sS[3][tx];
+    int32_t x_jj = 0, lost_f = 0;
+    if constexpr (kNormalise) {
+        if (j0 + tx < n_inputs) x_jj = np.x[(long long)f * P + pair_index(n_inputs, j0 + tx, j0 + tx)];
+        lost_f = np.lost[f];
+    }
     for (int ic = ty; ic < 32; ic += 8) {
         const int i = i0 + ic, j = j0 + tx;
         if (j < n_inputs && i <= j) {
@@ -94,7 +110,19 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
             uint32_t im;
             if (diag_super) im = (i == j) ? 0u : sQ[tx][ic] - sX[tx][ic] + 8u * (shi - sli) - 8u * (shj - slj);
             else im = sQ[tx][ic] - 7u * shi - 8u * sli - 8u * shj + 8u * slj;
-            *reinterpret_cast<int2 *>(out + ((long long)f * P + pair_index(n_inputs, i, j)) * 2) = make_int2((int32_t)re, (int32_t)im);
+            const long long p = (long long)f * P + pair_index(n_inputs, i, j);
+            if constexpr (kNormalise) {
+                // L = lost + c_i + c_j - X_ij (the point (i, i) receives its counter once); V~ = V * T / (T - L)
+                const int32_t x_ii = np.x[(long long)f * P + pair_index(n_inputs, i, i)];
+                const int32_t lost_ij = lost_f + x_ii + ((i != j) ? (x_jj - np.x[p]) : 0);
+                const int32_t valid = (int32_t)np.n_samples - lost_ij;
+                const float scale = (valid > 0) ? __fdiv_rn((float)np.n_samples, (float)valid) : 0.0f;
+                *reinterpret_cast<float2 *>(reinterpret_cast<float *>(out_v) + p * 2) =
+                    make_float2(__fmul_rn((float)(int32_t)re, scale), __fmul_rn((float)(int32_t)im, scale));
+                if (np.lost_out) np.lost_out[p] = lost_ij;
+            } else {
+                *reinterpret_cast<int2 *>(out + p * 2) = make_int2((int32_t)re, (int32_t)im);
+            }
         }
     }
 }

@@ -14,6 +14,7 @@
 
 #include "finalize_kernel.cuh"
 #include "layout.hpp"
+#include "normalise_kernel.cuh"
 #include "schedule.hpp"
 #include "xengine_kernel.cuh"
 
@@ -27,6 +28,7 @@ struct xcorr_handle {
     int n_inputs = 0, n_freq = 0, n_time = 0;
     int device = 0;
     int n_workers = 0;
+    int n_sms = 0;
     int n_tiles = 0;                 // F * n_supertiles
     bool offdiag = false;            // N > 256: kernel variant with the column block and -Im plane
     size_t frame_bytes = 0, output_bytes = 0, acc_bytes = 0;
@@ -44,6 +46,15 @@ struct xcorr_handle {
     uint64_t launches = 0;
     int last_cuda_error = 0;
     PFN_encodeTiled encode = nullptr;
+    // lost-sample normalisation (xcorr_norm_enable): flag-intersection accumulator, packet-loss counters
+    bool norm = false;
+    int32_t *flag_x = nullptr;       // device int32[F][P]
+    int32_t *lost_dev = nullptr;     // device int32[F]
+    int32_t *lost_pinned = nullptr;  // page-locked int32[F]: snapshot handed to the H2D copy of a read
+    long long *lost_acc = nullptr;   // host: lost samples per channel since the last read
+    int32_t *staging_lost = nullptr; // device int32[F][P] for host reads of the normalisation matrix
+    cudaEvent_t lost_copied = nullptr;
+    bool flags_dirty = false;        // flag_x holds counts of the current integration
 };
 
 struct xcorr_stream {
@@ -103,6 +114,12 @@ extern "C" void xcorr_destroy(xcorr_handle *h)
     cudaFree(h->segments);
     cudaFree(h->worker_begin);
     cudaFree(h->tile_slot_begin);
+    cudaFree(h->flag_x);
+    cudaFree(h->lost_dev);
+    cudaFree(h->staging_lost);
+    if (h->lost_pinned) cudaFreeHost(h->lost_pinned);
+    if (h->lost_copied) cudaEventDestroy(h->lost_copied);
+    delete[] h->lost_acc;
     delete h;
 }
 
@@ -130,6 +147,7 @@ extern "C" int xcorr_create(int n_inputs, int n_freq, int t_per_frame, xcorr_han
     const int nb = n_super(n_inputs);
     h->n_tiles = n_freq * n_supertiles(nb);
     h->offdiag = nb > 1;
+    h->n_sms = prop.multiProcessorCount;
     h->n_workers = prop.multiProcessorCount / 2;
     if (h->n_workers < 1) { delete h; return XCORR_EARCH; }
 
@@ -248,22 +266,40 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
     return XCORR_OK;
 }
 
-extern "C" int xcorr_read(xcorr_handle *h, int32_t *upper_triangle_out, void *cuda_stream)
+static bool is_device_pointer(const void *ptr)
 {
-    if (!h || !upper_triangle_out) return XCORR_EINVAL;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaPointerAttributes attr;
-    bool on_device = false;
-    if (cudaPointerGetAttributes(&attr, upper_triangle_out) == cudaSuccess)
-        on_device = (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged);
-    else
-        cudaGetLastError();
-    if (on_device && ((uintptr_t)upper_triangle_out & 15u) != 0) return XCORR_EINVAL;
-    int32_t *dst = on_device ? upper_triangle_out : h->staging;
+    if (cudaPointerGetAttributes(&attr, ptr) == cudaSuccess) return attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged;
+    cudaGetLastError();
+    return false;
+}
+
+// xcorr_read / xcorr_read_normalized: one launch of finalize_kernel; ends the integration
+static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *lost_matrix_out, void *cuda_stream)
+{
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const bool on_device = is_device_pointer(vis_out);
+    if (on_device && ((uintptr_t)vis_out & 15u) != 0) return XCORR_EINVAL;
+    void *dst = on_device ? vis_out : (void *)h->staging;
+    const bool lost_on_device = lost_matrix_out && is_device_pointer(lost_matrix_out);
+    int32_t *lost_dst = !lost_matrix_out ? nullptr : (lost_on_device ? lost_matrix_out : h->staging_lost);
     const int nt = (h->n_inputs + 31) / 32;
+    const size_t lost_matrix_bytes = h->output_bytes / 2;
     if (h->clean) {   // nothing integrated: the result is all zeros
         XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, s));
         XC_CUDA(h, cudaMemsetAsync(h->sums, 0, h->sums_bytes, s));
+    }
+    NormParams np = {};
+    if (normalise) {
+        // packet-loss counters: host accumulator -> page-locked snapshot -> device (the previous read's copy has long finished)
+        XC_CUDA(h, cudaEventSynchronize(h->lost_copied));
+        for (int f = 0; f < h->n_freq; ++f) h->lost_pinned[f] = (int32_t)h->lost_acc[f];
+        XC_CUDA(h, cudaMemcpyAsync(h->lost_dev, h->lost_pinned, sizeof(int32_t) * h->n_freq, cudaMemcpyHostToDevice, s));
+        XC_CUDA(h, cudaEventRecord(h->lost_copied, s));
+        np.x = h->flag_x;
+        np.lost = h->lost_dev;
+        np.lost_out = lost_dst;
+        np.n_samples = (uint32_t)h->samples_since_read;
     }
     {
         cudaLaunchAttribute attr[1];
@@ -275,20 +311,87 @@ extern "C" int xcorr_read(xcorr_handle *h, int32_t *upper_triangle_out, void *cu
         cfg.stream = s;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        XC_CUDA(h, cudaLaunchKernelEx(&cfg, finalize_kernel, (const int32_t *)h->acc, (const int32_t *)h->sums,
-                                      (const int32_t *)h->tile_slot_begin, dst, h->n_inputs, (uint32_t)h->offset_samples));
+        if (normalise)
+            XC_CUDA(h, cudaLaunchKernelEx(&cfg, finalize_kernel<true>, (const int32_t *)h->acc, (const int32_t *)h->sums,
+                                          (const int32_t *)h->tile_slot_begin, dst, h->n_inputs, (uint32_t)h->offset_samples, np));
+        else
+            XC_CUDA(h, cudaLaunchKernelEx(&cfg, finalize_kernel<false>, (const int32_t *)h->acc, (const int32_t *)h->sums,
+                                          (const int32_t *)h->tile_slot_begin, dst, h->n_inputs, (uint32_t)h->offset_samples, np));
     }
     XC_CUDA(h, cudaGetLastError());
     h->launches += 1;
-    // ends the integration: no clearing pass -- the next frame's epilogue overwrites its slots (first_frame)
+    // ends the integration: no clearing pass over the visibilities -- the next frame's epilogue overwrites its slots
     h->samples_since_read = 0;
     h->offset_samples = 0;
     h->clean = true;
-    if (!on_device) {
-        XC_CUDA(h, cudaMemcpyAsync(upper_triangle_out, h->staging, h->output_bytes, cudaMemcpyDeviceToHost, s));
-        XC_CUDA(h, cudaStreamSynchronize(s));
+    if (h->norm) {   // the flag / loss state belongs to the integration that just ended
+        if (h->flags_dirty) XC_CUDA(h, cudaMemsetAsync(h->flag_x, 0, lost_matrix_bytes, s));
+        h->flags_dirty = false;
+        for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] = 0;
+    }
+    if (!on_device) XC_CUDA(h, cudaMemcpyAsync(vis_out, h->staging, h->output_bytes, cudaMemcpyDeviceToHost, s));
+    if (lost_matrix_out && !lost_on_device)
+        XC_CUDA(h, cudaMemcpyAsync(lost_matrix_out, h->staging_lost, lost_matrix_bytes, cudaMemcpyDeviceToHost, s));
+    if (!on_device || (lost_matrix_out && !lost_on_device)) XC_CUDA(h, cudaStreamSynchronize(s));
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_read(xcorr_handle *h, int32_t *upper_triangle_out, void *cuda_stream)
+{
+    if (!h || !upper_triangle_out) return XCORR_EINVAL;
+    return read_common(h, upper_triangle_out, false, nullptr, cuda_stream);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// lost-sample normalisation (NEXT-1)
+// ---------------------------------------------------------------------------------------------------
+extern "C" int xcorr_norm_enable(xcorr_handle *h)
+{
+    if (!h) return XCORR_EINVAL;
+    if (h->norm) return XCORR_OK;
+    if (!h->clean) return XCORR_EINVAL;   // startup-time call: not in the middle of an integration
+    const size_t lost_matrix_bytes = h->output_bytes / 2;
+    cudaError_t e;
+    if ((e = cudaMalloc(&h->flag_x, lost_matrix_bytes)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
+    if ((e = cudaMalloc(&h->staging_lost, lost_matrix_bytes)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
+    if ((e = cudaMalloc(&h->lost_dev, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
+    if ((e = cudaMallocHost(&h->lost_pinned, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
+    h->lost_acc = new (std::nothrow) long long[h->n_freq]();
+    if (!h->lost_acc) return XCORR_ENOMEM;
+    XC_CUDA(h, cudaEventCreateWithFlags(&h->lost_copied, cudaEventDisableTiming));
+    XC_CUDA(h, cudaMemset(h->flag_x, 0, lost_matrix_bytes));
+    XC_CUDA(h, cudaMemset(h->lost_dev, 0, sizeof(int32_t) * h->n_freq));
+    h->norm = true;
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_norm_process(xcorr_handle *h, const uint8_t *flags_dev, const int32_t *lost_samples_host, void *cuda_stream)
+{
+    if (!h || !h->norm) return XCORR_EINVAL;
+    if (flags_dev && ((uintptr_t)flags_dev & 15u) != 0) return XCORR_EINVAL;
+    if (lost_samples_host) {
+        for (int f = 0; f < h->n_freq; ++f)
+            if (lost_samples_host[f] < 0 || lost_samples_host[f] > h->n_time) return XCORR_EINVAL;
+        for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] += lost_samples_host[f];
+    }
+    if (flags_dev) {
+        const unsigned long long n_bytes = (unsigned long long)h->frame_bytes / 8;
+        const unsigned long long n_chunks = (n_bytes + 15) / 16;
+        int blocks = h->n_sms * 8;     // grid-stride, 8 resident CTAs of 256 threads per SM
+        if ((unsigned long long)blocks * 256ull > n_chunks) blocks = (int)((n_chunks + 255) / 256);
+        flag_count_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>(flags_dev, n_bytes, h->n_inputs, h->n_freq, h->flag_x);
+        XC_CUDA(h, cudaGetLastError());
+        h->launches += 1;
+        h->flags_dirty = true;
     }
     return XCORR_OK;
+}
+
+extern "C" int xcorr_read_normalized(xcorr_handle *h, float *vis_out, int32_t *lost_matrix_out, void *cuda_stream)
+{
+    if (!h || !vis_out || !h->norm) return XCORR_EINVAL;
+    if (lost_matrix_out && is_device_pointer(lost_matrix_out) && ((uintptr_t)lost_matrix_out & 15u) != 0) return XCORR_EINVAL;
+    return read_common(h, vis_out, true, lost_matrix_out, cuda_stream);
 }
 
 // ---------------------------------------------------------------------------------------------------
