@@ -27,8 +27,9 @@ __device__ __forceinline__ uint4 slot_sum_v4(const int32_t *__restrict__ acc, in
 {
     uint4 s = make_uint4(0, 0, 0, 0);
     for (int sl = slot_begin; sl < slot_end; ++sl) {
-        const uint4 v = *reinterpret_cast<const uint4 *>(acc + (size_t)sl * kAccElemsPerSlot + (size_t)r * kAccElemsPerCta +
-                                                         ((size_t)col4 * kBlock + row) * 4);
+        // streaming (evict-first) load: a slot is dead once it has been read here
+        const uint4 v = __ldcs(reinterpret_cast<const uint4 *>(acc + (size_t)sl * kAccElemsPerSlot + (size_t)r * kAccElemsPerCta +
+                                                               ((size_t)col4 * kBlock + row) * 4));
         s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
     }
     return s;
@@ -121,7 +122,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
                     make_float2(__fmul_rn((float)(int32_t)re, scale), __fmul_rn((float)(int32_t)im, scale));
                 if (np.lost_out) np.lost_out[p] = lost_ij;
             } else {
-                *reinterpret_cast<int2 *>(out + p * 2) = make_int2((int32_t)re, (int32_t)im);
+                __stcs(reinterpret_cast<int2 *>(out + p * 2), make_int2((int32_t)re, (int32_t)im));
             }
         }
     }
