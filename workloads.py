@@ -186,3 +186,66 @@ def zero_lost_samples(frame: np.ndarray, flags: np.ndarray, lost_mask: np.ndarra
     out[flags] = 0
     out[lost_mask] = 0
     return out
+
+
+# ----------------------------------------------------------------------------------------------------------
+# UDP packets (NEXT-2).  Formatting and shuffling only: the assembly itself lives in the CUDA
+# path and, separately, in oracle/assembly.py.  Wire format = DESIGN.md section 13, reading P1.
+# ----------------------------------------------------------------------------------------------------------
+PACKET_MAGIC = 0x58454E47
+PACKET_HEADER_BYTES = 32
+
+
+def packetise(frame: np.ndarray, flag_bits: np.ndarray, seq0: int, s_per_packet: int = PACKET_T,
+              c_per_packet: int = PACKET_F) -> np.ndarray:
+    """Cut frame uint8[T][F][N] and its flag bit-field uint8[T][F][N/8] into packets, time-major then stream.
+
+    Returns uint8[n_packets][packet_bytes]: 32-byte header {u32 magic, u32 stream_id, u64 seq, 16 zero bytes},
+    payload uint8[S][C][N], footer uint8[S][C][N/8] (little endian).
+    """
+    T, F, N = frame.shape
+    S, C = s_per_packet, c_per_packet
+    assert T % S == 0 and F % C == 0 and flag_bits.shape == (T, F, N // 8)
+    nb, ns = T // S, F // C
+    pay = frame.reshape(nb, S, ns, C, N).transpose(0, 2, 1, 3, 4).reshape(nb * ns, S * C * N)
+    foot = flag_bits.reshape(nb, S, ns, C, N // 8).transpose(0, 2, 1, 3, 4).reshape(nb * ns, S * C * N // 8)
+    hdr = np.zeros((nb * ns, PACKET_HEADER_BYTES), dtype=np.uint8)
+    blk, stream = np.divmod(np.arange(nb * ns, dtype=np.uint64), np.uint64(ns))
+    hdr[:, 0:4] = np.full(nb * ns, PACKET_MAGIC, dtype="<u4").view(np.uint8).reshape(-1, 4)
+    hdr[:, 4:8] = stream.astype("<u4").view(np.uint8).reshape(-1, 4)
+    hdr[:, 8:16] = (np.uint64(seq0) + blk * np.uint64(S)).astype("<u8").view(np.uint8).reshape(-1, 8)
+    return np.ascontiguousarray(np.concatenate([hdr, pay, foot], axis=1))
+
+
+def disturb_packets(packets: np.ndarray, seed: int, p_loss: float = 2e-3, p_dup: float = 1e-3, p_late: float = 5e-3,
+                    max_delay: int = 40, n_foreign: int = 0) -> np.ndarray:
+    """A UDP network's effect on an in-order packet sequence ("lost, out of order, and duplicate
+    packets"): drop with p_loss, repeat with p_dup (the copy arrives a little later), delay with p_late by up to
+    max_delay positions, and insert n_foreign packets that do not belong (bad magic / stream / sequence number).
+    Returns the packets in ARRIVAL order, uint8[n_arrived][packet_bytes].
+    """
+    rng = np.random.default_rng(seed)
+    n = packets.shape[0]
+    keep = rng.random(n) >= p_loss
+    order_key = np.arange(n, dtype=np.float64)
+    late = rng.random(n) < p_late
+    order_key = order_key + late * rng.integers(1, max_delay + 1, n)
+    idx = np.nonzero(keep)[0]
+    key = order_key[idx]
+    dup = idx[rng.random(idx.size) < p_dup]
+    idx = np.concatenate([idx, dup])
+    key = np.concatenate([key, order_key[dup] + rng.integers(1, max_delay + 1, dup.size) + 0.5])
+    arrived = packets[idx[np.argsort(key, kind="stable")]].copy()
+    if n_foreign:
+        extra = packets[rng.integers(0, n, n_foreign)].copy()
+        for k in range(n_foreign):
+            kind = k % 3
+            if kind == 0:
+                extra[k, 0] ^= 0xFF                                  # wrong magic
+            elif kind == 1:
+                extra[k, 4:8] = np.array([0xFF, 0xFF, 0, 0], np.uint8)   # stream_id out of range
+            else:
+                extra[k, 8:16] = np.frombuffer(np.uint64(2 ** 40 + 1 + k).tobytes(), np.uint8)   # far-away, misaligned seq
+        pos = np.sort(rng.integers(0, arrived.shape[0] + 1, n_foreign))
+        arrived = np.insert(arrived, pos, extra, axis=0)
+    return np.ascontiguousarray(arrived)
