@@ -1,0 +1,112 @@
+/*
+ * xcorr_assemble.h -- C ABI of the packet -> frame assembly stage (libxcorr.so).
+ *
+ * What the paper's network threads do on the CPU (section II-A, :59-:81) as GPU kernels, directly
+ * upstream of xcorr_process():
+ *
+ *   "All that is required of the system is to place that data into the right location in a large host frame"
+ *
+ *   "all 256 inputs for one frequency take up 256 bytes.  For 8 frequency bands this represents 2KB. ... 4 time
+ *    samples are recorded in each packet.  The header contains a streamID that identifies which frequency bands
+ *    are represented in the packet, and a sequence number which gives the relative time"
+ *   "When the system detects packet loss, it writes zeros into the area of the GPU staging buffer where the
+ *    missing packet would have been placed. ... In the case of out of order packets, the sequence number is used
+ *    to copy the packet into the correct location.  Duplicate packets are simply ignored."
+ *   "The network threads track packet loss and F-engine error flags", the flags being
+ *   "bit-fields in the packet footers".
+ *
+ * Wire format of one packet (reading P1; Fig. 3 of the paper did not survive), little endian:
+ *
+ *     offset 0   u32 magic      = XCORR_PACKET_MAGIC
+ *            4   u32 stream_id    carries channels [C*stream_id, C*stream_id + C)
+ *            8   u64 seq          array-wide index of the packet's FIRST time sample (P2)
+ *           16   16 reserved bytes
+ *           32   payload uint8[S][C][N]      (input fastest: usable by the GPU unmodified)
+ *     32+S*C*N   footer  uint8[S][C][N/8]    flag bits, input n = bit (n % 8) of byte n / 8 (N1)
+ *
+ * S = samples per packet (4 in the paper), C = channels per stream (8), N = inputs (256): 9248 bytes ("~9K", :59).
+ * Packets lie back to back in ARRIVAL order in one buffer, packet k at byte k * xcorr_assembler_packet_bytes().
+ *
+ * Conventions as in xcorr.h: int return codes (XCORR_OK or a negative XCORR_E*), nothing allocated after create,
+ * no CPU fallback.
+ */
+#ifndef XCORR_ASSEMBLE_H_
+#define XCORR_ASSEMBLE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#include "xcorr.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define XCORR_PACKET_MAGIC        0x58454E47u
+#define XCORR_PACKET_HEADER_BYTES 32
+
+typedef struct xcorr_assembler xcorr_assembler;
+
+/*
+ * xcorr_assembler_create -- fix the shapes and allocate the position-ownership table and counters.
+ *
+ *   n_inputs, n_freq, t_per_frame   the frame shape uint8[T][F][N] of the xcorr handle this feeds
+ *   samples_per_packet  S > 0, T % S == 0
+ *   freq_per_packet     C > 0, F % C == 0, and C * N a multiple of 128 (rows of the payload and of the footer are
+ *                       then whole 16-byte vectors; true for the paper's C = 8 and any legal N)
+ * Errors: EINVAL, EARCH, ENOMEM, ECUDA.
+ */
+int xcorr_assembler_create(int n_inputs, int n_freq, int t_per_frame, int samples_per_packet, int freq_per_packet,
+                           xcorr_assembler **out);
+
+/* 32 + S*C*N + S*C*N/8.  0 for NULL. */
+size_t xcorr_assembler_packet_bytes(const xcorr_assembler *a);
+
+/*
+ * xcorr_assemble -- build ONE frame from the packets that arrived for it.  Asynchronous on `cuda_stream`.
+ *
+ *   packets     n_packets packets back to back in arrival order.  Any pointer the GPU can read: device memory, or
+ *               page-locked host memory (cudaHostAlloc / torch pin_memory -- the kernels then pull the packets over
+ *               PCIe themselves and no separate host-to-device copy of the ring is needed).  16-byte aligned.
+ *               BORROWED until `cuda_stream` has passed this call.  May be NULL if n_packets == 0.
+ *   seq0        sequence number of the frame's first time sample; the frame holds samples [seq0, seq0 + T).
+ *   frame_dev   OUT device uint8[T][F][N], 16-byte aligned: every position holds "good data or zeros";
+ *               the voltage byte of every flagged sample is zeroed as well (reading P5), so the frame
+ *               can go straight to xcorr_process().
+ *   flags_dev   OUT device uint8[T][F][N/8], 16-byte aligned: the flag bit-field in the layout xcorr_norm_process()
+ *               takes; zero where the packet is missing.  May be NULL.
+ *   lost_dev    OUT device int32[F]: time samples of each channel lost with their packets in this frame (the
+ *               paper's packet-loss counter, P6), ready for xcorr_norm_process_dev().  May be NULL.
+ *   counts_dev  OUT device uint32[4], may be NULL: {packets kept, duplicates ignored, packets rejected, positions
+ *               lost}.  A packet is rejected if its magic is wrong, its stream_id >= F / C, or its seq is outside
+ *               [seq0, seq0 + T) or not a multiple of S away from seq0 (P3: it belongs to another frame or stream).
+ *               Of several packets claiming one position the FIRST in arrival order is kept (P4).
+ *
+ * Two kernels: packet_claim_kernel (headers -> position ownership, lowest arrival index wins) and
+ * assemble_kernel (one pass over the positions: copy / zero-fill, flag masking, footers, loss counters).
+ * Errors: EINVAL (NULL / misaligned pointers, n_packets > 2^31 - 2), ECUDA.
+ */
+int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_packets, uint64_t seq0, void *frame_dev,
+                   uint8_t *flags_dev, int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream);
+
+/* Total number of this library's kernels launched through the assembler so far. */
+uint64_t xcorr_assembler_kernel_launches(const xcorr_assembler *a);
+
+/* Release everything (synchronises the device first).  NULL is a no-op. */
+void xcorr_assembler_destroy(xcorr_assembler *a);
+
+/*
+ * xcorr_norm_process_dev -- xcorr_norm_process() (xcorr.h) with the packet-loss counters on the DEVICE, so that the
+ * outputs of xcorr_assemble() feed the normalisation without a round trip through the host:
+ *
+ *   flags_dev          as in xcorr_norm_process (may be NULL)
+ *   lost_samples_dev   device int32[F], added on `cuda_stream` to the handle's per-channel counters (may be NULL);
+ *                      BORROWED until the stream has passed this call.
+ * Errors: EINVAL (normalisation not enabled, misaligned), ECUDA.
+ */
+int xcorr_norm_process_dev(xcorr_handle *h, const uint8_t *flags_dev, const int32_t *lost_samples_dev, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XCORR_ASSEMBLE_H_ */

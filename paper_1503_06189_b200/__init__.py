@@ -18,7 +18,9 @@ __all__ = [
     "xcorr_last_cuda_error", "xcorr_frame_bytes", "xcorr_output_bytes", "xcorr_kernel_launches",
     "xcorr_norm_enable", "xcorr_norm_process", "xcorr_read_normalized",
     "xcorr_stream_create", "xcorr_stream_submit", "xcorr_stream_sync", "xcorr_stream_read", "xcorr_stream_destroy",
-    "xcorr_debug_schedule", "xcorr_debug_stage_samples", "xcorr_debug_process_simt", "XCorr", "XCorrStream",
+    "xcorr_assembler_create", "xcorr_assembler_packet_bytes", "xcorr_assemble", "xcorr_assembler_kernel_launches",
+    "xcorr_assembler_destroy", "xcorr_norm_process_dev",
+    "xcorr_debug_schedule", "xcorr_debug_stage_samples", "xcorr_debug_process_simt", "XCorr", "XCorrStream", "Assembler",
 ]
 
 XCORR_OK, XCORR_EINVAL, XCORR_EARCH, XCORR_ENOMEM, XCORR_ECUDA, XCORR_EOVERFLOW = 0, -1, -2, -3, -4, -5
@@ -84,6 +86,18 @@ def lib() -> ctypes.CDLL:
     L.xcorr_stream_read.restype = ci
     L.xcorr_stream_destroy.argtypes = [vp]
     L.xcorr_stream_destroy.restype = None
+    L.xcorr_assembler_create.argtypes = [ci, ci, ci, ci, ci, ctypes.POINTER(vp)]
+    L.xcorr_assembler_create.restype = ci
+    L.xcorr_assembler_packet_bytes.argtypes = [vp]
+    L.xcorr_assembler_packet_bytes.restype = ctypes.c_size_t
+    L.xcorr_assemble.argtypes = [vp, vp, ctypes.c_size_t, ctypes.c_uint64, vp, vp, vp, vp, vp]
+    L.xcorr_assemble.restype = ci
+    L.xcorr_assembler_kernel_launches.argtypes = [vp]
+    L.xcorr_assembler_kernel_launches.restype = ctypes.c_uint64
+    L.xcorr_assembler_destroy.argtypes = [vp]
+    L.xcorr_assembler_destroy.restype = None
+    L.xcorr_norm_process_dev.argtypes = [vp, vp, vp, vp]
+    L.xcorr_norm_process_dev.restype = ci
     L.xcorr_debug_schedule.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ctypes.c_int32), ci, ctypes.POINTER(ctypes.c_int32)]
     L.xcorr_debug_schedule.restype = ci
     L.xcorr_debug_stage_samples.argtypes = []
@@ -144,6 +158,36 @@ def xcorr_norm_process(handle: int, flags_dev: int, lost_samples_host: int, cuda
 
 def xcorr_read_normalized(handle: int, vis_out: int, lost_matrix_out: int = 0, cuda_stream: int = 0) -> int:
     return lib().xcorr_read_normalized(handle, vis_out, lost_matrix_out or None, cuda_stream)
+
+
+def xcorr_norm_process_dev(handle: int, flags_dev: int, lost_samples_dev: int, cuda_stream: int = 0) -> int:
+    return lib().xcorr_norm_process_dev(handle, flags_dev or None, lost_samples_dev or None, cuda_stream)
+
+
+def xcorr_assembler_create(n_inputs: int, n_freq: int, t_per_frame: int, samples_per_packet: int = 4,
+                           freq_per_packet: int = 8) -> tuple[int, int]:
+    a = ctypes.c_void_p()
+    rc = lib().xcorr_assembler_create(int(n_inputs), int(n_freq), int(t_per_frame), int(samples_per_packet), int(freq_per_packet),
+                                      ctypes.byref(a))
+    return rc, (a.value or 0)
+
+
+def xcorr_assembler_packet_bytes(assembler: int) -> int:
+    return lib().xcorr_assembler_packet_bytes(assembler)
+
+
+def xcorr_assemble(assembler: int, packets: int, n_packets: int, seq0: int, frame_dev: int, flags_dev: int = 0, lost_dev: int = 0,
+                   counts_dev: int = 0, cuda_stream: int = 0) -> int:
+    return lib().xcorr_assemble(assembler, packets or None, int(n_packets), int(seq0), frame_dev or None, flags_dev or None,
+                                lost_dev or None, counts_dev or None, cuda_stream)
+
+
+def xcorr_assembler_kernel_launches(assembler: int) -> int:
+    return lib().xcorr_assembler_kernel_launches(assembler)
+
+
+def xcorr_assembler_destroy(assembler: int) -> None:
+    lib().xcorr_assembler_destroy(assembler)
 
 
 def xcorr_stream_create(handle: int, depth: int = 2) -> tuple[int, int]:
@@ -267,6 +311,16 @@ class XCorr:
             lptr = lost_samples.ctypes.data
         self._check(xcorr_norm_process(self.handle, fptr, lptr, _stream_handle(stream)), "xcorr_norm_process")
 
+    def norm_process_dev(self, flags_dev=None, lost_dev=None, stream=None) -> None:
+        """As norm_process with the packet-loss counters in a CUDA int32 tensor [F] (the output of Assembler.assemble)."""
+        fptr = flags_dev.data_ptr() if flags_dev is not None else 0
+        if flags_dev is not None and (not flags_dev.is_cuda or flags_dev.numel() * flags_dev.element_size() * 8 != self.frame_bytes):
+            raise ValueError("flags_dev must be a contiguous CUDA tensor of frame_bytes / 8 bytes")
+        if lost_dev is not None and (not lost_dev.is_cuda or lost_dev.numel() != self.n_freq or lost_dev.element_size() != 4):
+            raise ValueError("lost_dev must be a CUDA int32 tensor of n_freq elements")
+        lptr = lost_dev.data_ptr() if lost_dev is not None else 0
+        self._check(xcorr_norm_process_dev(self.handle, fptr, lptr, _stream_handle(stream)), "xcorr_norm_process_dev")
+
     def read_normalized(self, out=None, lost_out=None, stream=None):
         """-> float32[F][P][2] (allocated on the device if None); lost_out: optional int32[F][P] tensor for L."""
         import torch
@@ -325,6 +379,54 @@ class XCorrStream:
         if getattr(self, "stream", 0):
             xcorr_stream_destroy(self.stream)
             self.stream = 0
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Assembler:
+    """Packet -> frame assembly (NEXT-2, include/xcorr_assemble.h): packets in arrival order -> frame, flags, loss counters."""
+
+    def __init__(self, n_inputs: int, n_freq: int, t_per_frame: int, samples_per_packet: int = 4, freq_per_packet: int = 8):
+        rc, a = xcorr_assembler_create(n_inputs, n_freq, t_per_frame, samples_per_packet, freq_per_packet)
+        if rc != XCORR_OK:
+            raise XCorrError(rc, "xcorr_assembler_create")
+        self.handle = a
+        self.n_inputs, self.n_freq, self.t_per_frame = n_inputs, n_freq, t_per_frame
+        self.packet_bytes = xcorr_assembler_packet_bytes(a)
+
+    @property
+    def kernel_launches(self) -> int:
+        return xcorr_assembler_kernel_launches(self.handle)
+
+    def assemble(self, packets, n_packets: int, seq0: int, frame=None, flags=None, lost=None, counts=None, stream=None):
+        """packets: CUDA or pinned-CPU uint8 tensor holding >= n_packets packets back to back (arrival order).
+        frame / flags / lost / counts: CUDA output tensors (allocated if None).  -> (frame, flags, lost, counts)."""
+        import torch
+        if packets is not None and packets.numel() * packets.element_size() < n_packets * self.packet_bytes:
+            raise ValueError("packets holds fewer than n_packets packets")
+        if packets is not None and not packets.is_cuda and not packets.is_pinned():
+            raise ValueError("host packets must be page-locked (pin_memory) so the GPU can read them")
+        t, f, n = self.t_per_frame, self.n_freq, self.n_inputs
+        frame = torch.empty((t, f, n), dtype=torch.uint8, device="cuda") if frame is None else frame
+        flags = torch.empty((t, f, n // 8), dtype=torch.uint8, device="cuda") if flags is None else flags
+        lost = torch.empty(f, dtype=torch.int32, device="cuda") if lost is None else lost
+        counts = torch.empty(4, dtype=torch.int32, device="cuda") if counts is None else counts
+        if frame.numel() != t * f * n or flags.numel() * 8 != t * f * n or lost.numel() != f or counts.numel() != 4:
+            raise ValueError("output tensor of the wrong size")
+        rc = xcorr_assemble(self.handle, packets.data_ptr() if packets is not None else 0, n_packets, seq0, frame.data_ptr(),
+                            flags.data_ptr(), lost.data_ptr(), counts.data_ptr(), _stream_handle(stream))
+        if rc != XCORR_OK:
+            raise XCorrError(rc, "xcorr_assemble")
+        return frame, flags, lost, counts
+
+    def close(self) -> None:
+        if getattr(self, "handle", 0):
+            xcorr_assembler_destroy(self.handle)
+            self.handle = 0
 
     def __del__(self):
         try:

@@ -1,0 +1,147 @@
+// assemble_kernel.cuh -- packet -> frame assembly (SURVEY.md 8(f) NEXT-2; section II-A, :59-:81).
+//
+// The paper's network threads place each UDP payload "into the right location in a large host frame" (:65) by its
+// sequence number, write zeros where a packet is missing, and ignore duplicates (:81).  Here that is two kernels over
+// the packets as they arrived (wire format: include/xcorr_assemble.h, P1):
+//
+//   packet_claim_kernel   one thread per packet: parse the header, reject what is not of this frame (P3), and claim the
+//                         packet's position (time block, stream) with atomicMin(arrival index) -- the first arrival
+//                         wins whatever the order in which threads run (P4), out-of-order packets need nothing else.
+//   assemble_kernel       one pass over the POSITIONS of the frame (grid-stride, one CTA per position at a time): copy
+//                         the owner's payload as 16-byte vectors into the S rows of the frame, zeroing the byte of every
+//                         flagged sample (P5) -- the footer is "read initially as 32-bit integers, and bit-field
+//                         extraction is performed only if ... non-zero": here 16 flag bits per 16 voltage
+//                         bytes, expanded only when non-zero; copy the footer into the frame's flag bit-field; where no
+//                         packet owns the position write zeros ("good data or zeros in every location", :81) and add S to
+//                         the channels' packet-loss counters (:113, P6).  Every byte of the frame and of the flag field
+//                         is written exactly once: no clearing pass.
+//
+// HBM-bound: per frame, reads n_packets * packet_bytes, writes T*F*N + T*F*N/8.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace xc {
+
+constexpr uint32_t kPacketMagic = 0x58454E47u;
+constexpr int kPacketHeaderBytes = 32;
+constexpr uint32_t kNoOwner = 0xFFFFFFFFu;
+
+struct AssembleShape {
+    int n_inputs, n_freq, n_time;   // N, F, T
+    int s_per_packet, c_per_packet; // S, C
+    int n_streams, n_blocks;        // F / C, T / S
+    unsigned long long packet_bytes;
+};
+
+// counts[0] kept  [1] duplicates  [2] rejected  [3] positions lost  [4] valid (scratch)  [5] CTA ticket (scratch)
+__global__ void __launch_bounds__(256) packet_claim_kernel(const uint8_t *__restrict__ packets, unsigned int n_packets,
+                                                            unsigned long long seq0, AssembleShape sh, uint32_t *__restrict__ owner,
+                                                            uint32_t *__restrict__ counts)
+{
+    const unsigned int k = blockIdx.x * blockDim.x + threadIdx.x;
+    bool valid = false, rejected = false;
+    if (k < n_packets) {
+        const uint4 hdr = __ldg(reinterpret_cast<const uint4 *>(packets + (unsigned long long)k * sh.packet_bytes));
+        const uint32_t magic = hdr.x, stream = hdr.y;
+        const unsigned long long seq = (unsigned long long)hdr.z | ((unsigned long long)hdr.w << 32);
+        const unsigned long long dt = seq - seq0;     // wraps for seq < seq0 -> fails the range test
+        valid = magic == kPacketMagic && stream < (uint32_t)sh.n_streams && seq >= seq0 && dt < (unsigned long long)sh.n_time &&
+                dt % (unsigned)sh.s_per_packet == 0;
+        rejected = !valid;
+        if (valid) atomicMin(owner + (dt / (unsigned)sh.s_per_packet) * (unsigned)sh.n_streams + stream, k);
+    }
+    // warp-aggregated counters
+    const unsigned v = __ballot_sync(0xFFFFFFFFu, valid), r = __ballot_sync(0xFFFFFFFFu, rejected);
+    if ((threadIdx.x & 31) == 0) {
+        if (v) atomicAdd(counts + 4, __popc(v));
+        if (r) atomicAdd(counts + 2, __popc(r));
+    }
+}
+
+// 4 flag bits -> 4 byte masks (0xFF where flagged): bit k of x goes to bit 8k (the partial products never collide)
+__device__ __forceinline__ uint32_t spread4(uint32_t x) { return (((x & 0xFu) * 0x00204081u) & 0x01010101u) * 0xFFu; }
+
+__global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict__ packets, AssembleShape sh,
+                                                        const uint32_t *__restrict__ owner, uint8_t *__restrict__ frame,
+                                                        uint8_t *__restrict__ flags, int32_t *__restrict__ lost, uint32_t *__restrict__ counts)
+{
+    const int N = sh.n_inputs, F = sh.n_freq, S = sh.s_per_packet, C = sh.c_per_packet;
+    const unsigned row_chunks = (unsigned)(C * N) >> 4;            // 16-byte vectors per time sample of one stream
+    const unsigned pay_chunks = row_chunks * (unsigned)S;
+    const unsigned frow_chunks = (unsigned)(C * N) >> 7;           // same for the flag bit-field (C*N/8 bytes per sample)
+    const unsigned foot_chunks = frow_chunks * (unsigned)S;
+    const unsigned long long pay_bytes = (unsigned long long)S * C * N;
+    const unsigned n_pos = (unsigned)sh.n_blocks * (unsigned)sh.n_streams;
+    uint32_t kept_local = 0, lost_local = 0;                      // thread 0's tallies of this CTA
+    for (unsigned pos = blockIdx.x; pos < n_pos; pos += gridDim.x) {
+        const unsigned blk = pos / (unsigned)sh.n_streams, stream = pos % (unsigned)sh.n_streams;
+        const uint32_t own = __ldg(owner + pos);
+        // byte offset of (t = blk*S, f = C*stream, n = 0) in the frame; rows of one stream are C*N contiguous bytes, F*N apart
+        const unsigned long long f0 = ((unsigned long long)blk * S * F + (unsigned long long)C * stream) * (unsigned long long)N;
+        uint4 *frame_v = reinterpret_cast<uint4 *>(frame + f0);
+        const unsigned long long frame_row_stride = ((unsigned long long)F * N) >> 4;   // in uint4
+        if (own != kNoOwner) {
+            const uint8_t *pkt = packets + (unsigned long long)own * sh.packet_bytes;
+            const uint4 *pay = reinterpret_cast<const uint4 *>(pkt + kPacketHeaderBytes);
+            const uint16_t *foot16 = reinterpret_cast<const uint16_t *>(pkt + kPacketHeaderBytes + pay_bytes);
+            for (unsigned c = threadIdx.x; c < pay_chunks; c += blockDim.x) {
+                uint4 v = __ldg(pay + c);
+                const uint32_t bits = __ldg(foot16 + c);           // the 16 flag bits of these 16 inputs
+                if (bits) {                                        // rare: zero the flagged samples' bytes (P5)
+                    v.x &= ~spread4(bits);
+                    v.y &= ~spread4(bits >> 4);
+                    v.z &= ~spread4(bits >> 8);
+                    v.w &= ~spread4(bits >> 12);
+                }
+                const unsigned dt = c / row_chunks, w = c - dt * row_chunks;
+                frame_v[dt * frame_row_stride + w] = v;
+            }
+            if (flags) {
+                const uint4 *foot = reinterpret_cast<const uint4 *>(foot16);
+                uint4 *flags_v = reinterpret_cast<uint4 *>(flags + (f0 >> 3));
+                for (unsigned c = threadIdx.x; c < foot_chunks; c += blockDim.x) {
+                    const unsigned dt = c / frow_chunks, w = c - dt * frow_chunks;
+                    flags_v[dt * (frame_row_stride >> 3) + w] = __ldg(foot + c);
+                }
+            }
+            kept_local += 1;
+        } else {
+            // "it writes zeros into the area of the GPU staging buffer where the missing packet would have been placed" (:81)
+            const uint4 z = make_uint4(0, 0, 0, 0);
+            for (unsigned c = threadIdx.x; c < pay_chunks; c += blockDim.x) {
+                const unsigned dt = c / row_chunks, w = c - dt * row_chunks;
+                frame_v[dt * frame_row_stride + w] = z;
+            }
+            if (flags) {
+                uint4 *flags_v = reinterpret_cast<uint4 *>(flags + (f0 >> 3));
+                for (unsigned c = threadIdx.x; c < foot_chunks; c += blockDim.x) {
+                    const unsigned dt = c / frow_chunks, w = c - dt * frow_chunks;
+                    flags_v[dt * (frame_row_stride >> 3) + w] = z;
+                }
+            }
+            if (lost && threadIdx.x < (unsigned)C) atomicAdd(lost + C * stream + threadIdx.x, S);   // packet-loss counter (P6)
+            lost_local += 1;
+        }
+    }
+    // packet counts: one atomic per CTA; the last CTA to finish derives duplicates = valid - kept
+    if (counts && threadIdx.x == 0) {
+        if (kept_local) atomicAdd(counts + 0, kept_local);
+        if (lost_local) atomicAdd(counts + 3, lost_local);
+        __threadfence();
+        if (atomicAdd(counts + 5, 1u) == gridDim.x - 1) {
+            __threadfence();
+            const uint32_t kept = atomicAdd(counts + 0, 0u), valid = atomicAdd(counts + 4, 0u);
+            counts[1] = valid - kept;
+        }
+    }
+}
+
+// lost-sample counters of one frame, device -> the handle's device accumulator (xcorr_norm_process_dev)
+__global__ void lost_add_kernel(const int32_t *__restrict__ lost_frame, int32_t *__restrict__ lost_acc, int n_freq)
+{
+    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f < n_freq) lost_acc[f] += lost_frame[f];
+}
+
+}  // namespace xc

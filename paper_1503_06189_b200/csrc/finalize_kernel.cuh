@@ -39,6 +39,7 @@ __device__ __forceinline__ uint4 slot_sum_v4(const int32_t *__restrict__ acc, in
 struct NormParams {
     const int32_t *x;        // device int32[F][P]: flag intersections, diagonal = flag counters
     const int32_t *lost;     // device int32[F]: time samples lost with their packets, per channel
+    const int32_t *lost_extra;  // device int32[F]: the same, counted on the device (xcorr_norm_process_dev); added to `lost`
     int32_t *lost_out;       // device int32[F][P] or nullptr: the normalisation matrix L itself
     uint32_t n_samples;      // T: samples integrated since the last read
 };
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
     int32_t x_jj = 0, lost_f = 0;
     if constexpr (kNormalise) {
         if (j0 + tx < n_inputs) x_jj = np.x[(long long)f * P + pair_index(n_inputs, j0 + tx, j0 + tx)];
-        lost_f = np.lost[f];
+        lost_f = np.lost[f] + np.lost_extra[f];
     }
     for (int ic = ty; ic < 32; ic += 8) {
         const int i = i0 + ic, j = j0 + tx;

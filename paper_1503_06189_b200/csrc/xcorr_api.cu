@@ -12,6 +12,8 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include "../../include/xcorr_assemble.h"
+#include "assemble_kernel.cuh"
 #include "finalize_kernel.cuh"
 #include "layout.hpp"
 #include "normalise_kernel.cuh"
@@ -50,6 +52,8 @@ struct xcorr_handle {
     bool norm = false;
     int32_t *flag_x = nullptr;       // device int32[F][P]
     int32_t *lost_dev = nullptr;     // device int32[F]
+    int32_t *lost_dev_acc = nullptr; // device int32[F]: counters added on the device (xcorr_norm_process_dev)
+    bool lost_dev_dirty = false;
     int32_t *lost_pinned = nullptr;  // page-locked int32[F]: snapshot handed to the H2D copy of a read
     long long *lost_acc = nullptr;   // host: lost samples per channel since the last read
     int32_t *staging_lost = nullptr; // device int32[F][P] for host reads of the normalisation matrix
@@ -116,6 +120,7 @@ extern "C" void xcorr_destroy(xcorr_handle *h)
     cudaFree(h->tile_slot_begin);
     cudaFree(h->flag_x);
     cudaFree(h->lost_dev);
+    cudaFree(h->lost_dev_acc);
     cudaFree(h->staging_lost);
     if (h->lost_pinned) cudaFreeHost(h->lost_pinned);
     if (h->lost_copied) cudaEventDestroy(h->lost_copied);
@@ -298,6 +303,7 @@ static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *
         XC_CUDA(h, cudaEventRecord(h->lost_copied, s));
         np.x = h->flag_x;
         np.lost = h->lost_dev;
+        np.lost_extra = h->lost_dev_acc;
         np.lost_out = lost_dst;
         np.n_samples = (uint32_t)h->samples_since_read;
     }
@@ -327,6 +333,8 @@ static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *
     if (h->norm) {   // the flag / loss state belongs to the integration that just ended
         if (h->flags_dirty) XC_CUDA(h, cudaMemsetAsync(h->flag_x, 0, lost_matrix_bytes, s));
         h->flags_dirty = false;
+        if (h->lost_dev_dirty) XC_CUDA(h, cudaMemsetAsync(h->lost_dev_acc, 0, sizeof(int32_t) * h->n_freq, s));
+        h->lost_dev_dirty = false;
         for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] = 0;
     }
     if (!on_device) XC_CUDA(h, cudaMemcpyAsync(vis_out, h->staging, h->output_bytes, cudaMemcpyDeviceToHost, s));
@@ -355,14 +363,31 @@ extern "C" int xcorr_norm_enable(xcorr_handle *h)
     if ((e = cudaMalloc(&h->flag_x, lost_matrix_bytes)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
     if ((e = cudaMalloc(&h->staging_lost, lost_matrix_bytes)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
     if ((e = cudaMalloc(&h->lost_dev, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
+    if ((e = cudaMalloc(&h->lost_dev_acc, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
     if ((e = cudaMallocHost(&h->lost_pinned, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
     h->lost_acc = new (std::nothrow) long long[h->n_freq]();
     if (!h->lost_acc) return XCORR_ENOMEM;
     XC_CUDA(h, cudaEventCreateWithFlags(&h->lost_copied, cudaEventDisableTiming));
     XC_CUDA(h, cudaMemset(h->flag_x, 0, lost_matrix_bytes));
     XC_CUDA(h, cudaMemset(h->lost_dev, 0, sizeof(int32_t) * h->n_freq));
+    XC_CUDA(h, cudaMemset(h->lost_dev_acc, 0, sizeof(int32_t) * h->n_freq));
     h->norm = true;
     return XCORR_OK;
+}
+
+static int launch_flag_count(xcorr_handle *h, const uint8_t *flags_dev, void *cuda_stream);
+
+extern "C" int xcorr_norm_process_dev(xcorr_handle *h, const uint8_t *flags_dev, const int32_t *lost_samples_dev, void *cuda_stream)
+{
+    if (!h || !h->norm) return XCORR_EINVAL;
+    if (flags_dev && ((uintptr_t)flags_dev & 15u) != 0) return XCORR_EINVAL;
+    if (lost_samples_dev) {
+        lost_add_kernel<<<(h->n_freq + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(lost_samples_dev, h->lost_dev_acc, h->n_freq);
+        XC_CUDA(h, cudaGetLastError());
+        h->launches += 1;
+        h->lost_dev_dirty = true;
+    }
+    return launch_flag_count(h, flags_dev, cuda_stream);
 }
 
 extern "C" int xcorr_norm_process(xcorr_handle *h, const uint8_t *flags_dev, const int32_t *lost_samples_host, void *cuda_stream)
@@ -374,6 +399,11 @@ extern "C" int xcorr_norm_process(xcorr_handle *h, const uint8_t *flags_dev, con
             if (lost_samples_host[f] < 0 || lost_samples_host[f] > h->n_time) return XCORR_EINVAL;
         for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] += lost_samples_host[f];
     }
+    return launch_flag_count(h, flags_dev, cuda_stream);
+}
+
+static int launch_flag_count(xcorr_handle *h, const uint8_t *flags_dev, void *cuda_stream)
+{
     if (flags_dev) {
         const unsigned long long n_bytes = (unsigned long long)h->frame_bytes / 8;
         const unsigned long long n_chunks = (n_bytes + 15) / 16;
@@ -517,3 +547,92 @@ extern "C" int xcorr_debug_read_profile(unsigned long long *out)
     return cudaMemcpyFromSymbol(out, g_prof, sizeof(unsigned long long) * 1024 * 16) == cudaSuccess ? XCORR_OK : XCORR_ECUDA;
 }
 #endif
+
+// ---------------------------------------------------------------------------------------------------
+// packet -> frame assembly (NEXT-2; include/xcorr_assemble.h)
+// ---------------------------------------------------------------------------------------------------
+struct xcorr_assembler {
+    AssembleShape sh = {};
+    int device = 0, n_sms = 0;
+    unsigned n_positions = 0;
+    uint32_t *owner = nullptr;     // device uint32[n_positions]: arrival index of the packet that owns the position
+    uint32_t *counts = nullptr;    // device uint32[8], see assemble_kernel.cuh
+    uint64_t launches = 0;
+    int last_cuda_error = 0;
+};
+
+extern "C" void xcorr_assembler_destroy(xcorr_assembler *a)
+{
+    if (!a) return;
+    cudaSetDevice(a->device);
+    cudaDeviceSynchronize();
+    cudaFree(a->owner);
+    cudaFree(a->counts);
+    delete a;
+}
+
+extern "C" size_t xcorr_assembler_packet_bytes(const xcorr_assembler *a) { return a ? (size_t)a->sh.packet_bytes : 0; }
+extern "C" uint64_t xcorr_assembler_kernel_launches(const xcorr_assembler *a) { return a ? a->launches : 0; }
+
+extern "C" int xcorr_assembler_create(int n_inputs, int n_freq, int t_per_frame, int samples_per_packet, int freq_per_packet,
+                                      xcorr_assembler **out)
+{
+    if (!out) return XCORR_EINVAL;
+    *out = nullptr;
+    int rc = validate_shape(n_inputs, n_freq, t_per_frame);
+    if (rc != XCORR_OK) return rc;
+    const int S = samples_per_packet, C = freq_per_packet;
+    if (S <= 0 || C <= 0 || t_per_frame % S != 0 || n_freq % C != 0) return XCORR_EINVAL;
+    if (((long long)C * n_inputs) % 128 != 0) return XCORR_EINVAL;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return XCORR_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return XCORR_ECUDA;
+    if (prop.major != 10) return XCORR_EARCH;
+    xcorr_assembler *a = new (std::nothrow) xcorr_assembler;
+    if (!a) return XCORR_ENOMEM;
+    a->device = dev;
+    a->n_sms = prop.multiProcessorCount;
+    a->sh.n_inputs = n_inputs; a->sh.n_freq = n_freq; a->sh.n_time = t_per_frame;
+    a->sh.s_per_packet = S; a->sh.c_per_packet = C;
+    a->sh.n_streams = n_freq / C; a->sh.n_blocks = t_per_frame / S;
+    const unsigned long long pay = (unsigned long long)S * C * n_inputs;
+    a->sh.packet_bytes = kPacketHeaderBytes + pay + pay / 8;
+    a->n_positions = (unsigned)a->sh.n_streams * (unsigned)a->sh.n_blocks;
+    cudaError_t e;
+    if ((e = cudaMalloc(&a->owner, sizeof(uint32_t) * (size_t)a->n_positions)) != cudaSuccess ||
+        (e = cudaMalloc(&a->counts, sizeof(uint32_t) * 8)) != cudaSuccess) {
+        cudaGetLastError();
+        xcorr_assembler_destroy(a);
+        return e == cudaErrorMemoryAllocation ? XCORR_ENOMEM : XCORR_ECUDA;
+    }
+    *out = a;
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_packets, uint64_t seq0, void *frame_dev,
+                              uint8_t *flags_dev, int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream)
+{
+    if (!a || !frame_dev || (!packets && n_packets) || n_packets > 0x7FFFFFFEull) return XCORR_EINVAL;
+    if (((uintptr_t)packets & 15u) || ((uintptr_t)frame_dev & 15u) || ((uintptr_t)flags_dev & 15u) || ((uintptr_t)lost_dev & 3u) ||
+        ((uintptr_t)counts_dev & 3u))
+        return XCORR_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    XC_CUDA(a, cudaMemsetAsync(a->owner, 0xFF, sizeof(uint32_t) * (size_t)a->n_positions, s));
+    XC_CUDA(a, cudaMemsetAsync(a->counts, 0, sizeof(uint32_t) * 8, s));
+    if (lost_dev) XC_CUDA(a, cudaMemsetAsync(lost_dev, 0, sizeof(int32_t) * a->sh.n_freq, s));
+    if (n_packets) {
+        packet_claim_kernel<<<(unsigned)((n_packets + 255) / 256), 256, 0, s>>>((const uint8_t *)packets, (unsigned)n_packets, seq0, a->sh,
+                                                                               a->owner, a->counts);
+        XC_CUDA(a, cudaGetLastError());
+        a->launches += 1;
+    }
+    // grid-stride over the positions: 8 resident CTAs of 256 threads per SM
+    unsigned blocks = (unsigned)a->n_sms * 8u;
+    if (blocks > a->n_positions) blocks = a->n_positions;
+    assemble_kernel<<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, a->owner, (uint8_t *)frame_dev, flags_dev, lost_dev, a->counts);
+    XC_CUDA(a, cudaGetLastError());
+    a->launches += 1;
+    if (counts_dev) XC_CUDA(a, cudaMemcpyAsync(counts_dev, a->counts, sizeof(uint32_t) * 4, cudaMemcpyDefault, s));
+    return XCORR_OK;
+}

@@ -64,6 +64,21 @@ def test_null_handles_are_harmless():
     assert xb.xcorr_stream_submit(0, 0) == xb.XCORR_EINVAL
 
 
+@pytest.mark.parametrize("args", [(16, 8, 16, 0, 8), (16, 8, 16, 4, 0), (16, 8, 18, 4, 8), (16, 12, 16, 4, 8), (16, 8, 16, 4, 4),
+                                  (24, 8, 16, 4, 8)])
+def test_assembler_create_rejects_bad_shapes_without_touching_the_gpu(args):
+    rc, a = xb.xcorr_assembler_create(*args)
+    assert rc == xb.XCORR_EINVAL and a == 0
+
+
+def test_assembler_null_handles_are_harmless():
+    assert xb.xcorr_assembler_packet_bytes(0) == 0
+    assert xb.xcorr_assembler_kernel_launches(0) == 0
+    xb.xcorr_assembler_destroy(0)
+    assert xb.xcorr_assemble(0, 0, 0, 0, 0) == xb.XCORR_EINVAL
+    assert xb.xcorr_norm_process_dev(0, 0, 0, 0) == xb.XCORR_EINVAL
+
+
 def test_create_fails_loudly_without_a_gpu():
     try:
         import torch
