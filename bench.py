@@ -113,6 +113,62 @@ def oracle_sample(cfg: wl.Config, seconds_hint: float = 12.0):
             "cmac_per_s": cmacs / dt, "seconds": dt}
 
 
+def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
+    """NEXT-2 packet assembly and NEXT-1 lost-sample normalisation on the same frame shape: per-kernel CUDA-event times and
+    achieved HBM GB/s against the measured copy bandwidth (both are HBM-bound; algorithmic bytes as stated in DESIGN.md)."""
+    n, f, t = cfg.n_inputs, cfg.n_freq, cfg.n_time
+    fb = wl.sparse_flag_bits(n, f, t, 99)
+    pk = wl.packetise(host_frame, fb, 10 ** 12)
+    arrived = wl.disturb_packets(pk, 98, p_loss=2e-3, p_dup=1e-3, p_late=5e-3, n_foreign=16)
+    n_pk, pbytes = arrived.shape
+    pk_dev = [torch.from_numpy(arrived.reshape(-1)).cuda(), torch.from_numpy(arrived.reshape(-1).copy()).cuda()]
+    del pk, arrived
+    a = xb.Assembler(n, f, t)
+    x.norm_enable()
+    frame = torch.empty((t, f, n), dtype=torch.uint8, device="cuda")
+    flags = torch.empty((t, f, n // 8), dtype=torch.uint8, device="cuda")
+    lost = torch.empty(f, dtype=torch.int32, device="cuda")
+    counts = torch.empty(4, dtype=torch.int32, device="cuda")
+    vis = torch.empty((f, cfg.n_pairs, 2), dtype=torch.float32, device="cuda")
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    names = ["assemble", "process", "norm_process", "read_normalized"]
+    times = {k: [] for k in names}
+    for r in range(reps + 3):
+        e = [ev() for _ in range(5)]
+        with torch.cuda.stream(st):
+            e[0].record(st)
+            a.assemble(pk_dev[r % 2], n_pk, 10 ** 12, frame, flags, lost, counts, stream=st)
+            e[1].record(st)
+            x.process(frame, st)
+            e[2].record(st)
+            x.norm_process_dev(flags, lost, st)
+            e[3].record(st)
+            x.read_normalized(vis, stream=st)
+            e[4].record(st)
+        torch.cuda.synchronize()
+        if r >= 3:
+            for k, nm in enumerate(names):
+                times[nm].append(e[k].elapsed_time(e[k + 1]) * 1e3)
+    c = counts.cpu().tolist()
+    a.close()
+    us = {k: statistics.mean(v) for k, v in times.items()}
+    asm_bytes = n_pk * pbytes + cfg.frame_bytes + cfg.frame_bytes // 8
+    flag_bytes = cfg.frame_bytes // 8
+    return {
+        "what": "packets (arrival order, device resident) -> xcorr_assemble -> xcorr_process -> xcorr_norm_process_dev -> "
+                "xcorr_read_normalized; per-call CUDA-event means over %d repetitions" % reps,
+        "packets": n_pk, "packet_bytes": pbytes, "kept_dup_rejected_lostpos": c, "us": us,
+        "assemble_roofline": {"bound": "hbm", "achieved": asm_bytes / (us["assemble"] * 1e-6) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                              "frac": asm_bytes / (us["assemble"] * 1e-6) / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": asm_bytes,
+                              "note": "2 kernels (packet_claim_kernel + assemble_kernel) and 3 small memsets in the timed call"},
+        "flag_count_roofline": {"bound": "hbm", "achieved": flag_bytes / (us["norm_process"] * 1e-6) / 1e9, "peak": peaks["hbm_gbs"],
+                                "unit": "GB/s", "frac": flag_bytes / (us["norm_process"] * 1e-6) / 1e9 / peaks["hbm_gbs"],
+                                "algorithmic_bytes": flag_bytes,
+                                "note": "flag_count_kernel + lost_add_kernel; the flag field was just written, so part of it is an L2 hit"},
+        "pipeline_gbps": 8.0 * cfg.frame_bytes / (sum(us.values()) * 1e-6) / 1e9,
+    }
+
+
 def run_reference(args, cfg):
     """--impl reference: the oracle timed on the host cores, bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -146,6 +202,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-next-rows", action="store_true")
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
     if args.impl == "reference":
@@ -287,6 +344,11 @@ def main():
                "h2d_only_gbps": h2d_gbps, "paper_rate_gbps": 819.2 if cfg.name == "C3" else None}
         s.close()
 
+    # ---- the rows SURVEY.md 8(f) marks "next", same frame shape, timed one by one with CUDA events (not part of `value`)
+    next_rows = None
+    if rank == 0 and world == 1 and not args.no_next_rows and cfg.n_freq % wl.PACKET_F == 0 and cfg.n_time % wl.PACKET_T == 0:
+        next_rows = measure_next_rows(cfg, x, xb, torch, st, host_frames[0], peaks)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = oracle_sample(cfg)
@@ -305,7 +367,7 @@ def main():
             "pct_int8_peak_nominal": 100.0 * 8.0 * cmac_per_s / world / (NOMINAL_INT8_TOPS * 1e12),
             "pct_int8_peak_measured": 100.0 * 8.0 * cmac_per_s / world / (peak * 1e12),
             "paper_context": "51.2 Gb/s per 3-GPU server, 819.2 Gb/s over 16 servers (PAPER.md Table I; other hardware)",
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "next_rows": next_rows, "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
     x.close()

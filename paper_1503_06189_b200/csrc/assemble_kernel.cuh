@@ -144,4 +144,16 @@ __global__ void lost_add_kernel(const int32_t *__restrict__ lost_frame, int32_t 
     if (f < n_freq) lost_acc[f] += lost_frame[f];
 }
 
+// xcorr_read_normalized: this integration's packet-loss counters = the host-counted snapshot (page-locked, read in place)
+// + the device-counted ones, which start again from zero
+__global__ void lost_gather_kernel(const int32_t *__restrict__ snapshot_host, int32_t *__restrict__ lost_acc, int32_t *__restrict__ lost_out,
+                                   int n_freq)
+{
+    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f < n_freq) {
+        lost_out[f] = snapshot_host[f] + lost_acc[f];
+        lost_acc[f] = 0;
+    }
+}
+
 }  // namespace xc

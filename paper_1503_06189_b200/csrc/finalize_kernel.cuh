@@ -37,9 +37,9 @@ __device__ __forceinline__ uint4 slot_sum_v4(const int32_t *__restrict__ acc, in
 
 // Lost-sample normalisation fused into the write (normalise_kernel.cuh): inputs of the kNormalise variant
 struct NormParams {
-    const int32_t *x;        // device int32[F][P]: flag intersections, diagonal = flag counters
+    int32_t *x;              // device int32[F][P]: flag intersections, diagonal = flag counters; the intersections are
+                             // cleared here as they are read (each by exactly one thread), the diagonal by clear_diag_kernel
     const int32_t *lost;     // device int32[F]: time samples lost with their packets, per channel
-    const int32_t *lost_extra;  // device int32[F]: the same, counted on the device (xcorr_norm_process_dev); added to `lost`
     int32_t *lost_out;       // device int32[F][P] or nullptr: the normalisation matrix L itself
     uint32_t n_samples;      // T: samples integrated since the last read
 };
@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
     int32_t x_jj = 0, lost_f = 0;
     if constexpr (kNormalise) {
         if (j0 + tx < n_inputs) x_jj = np.x[(long long)f * P + pair_index(n_inputs, j0 + tx, j0 + tx)];
-        lost_f = np.lost[f] + np.lost_extra[f];
+        lost_f = np.lost[f];
     }
     for (int ic = ty; ic < 32; ic += 8) {
         const int i = i0 + ic, j = j0 + tx;
@@ -116,7 +116,12 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
             if constexpr (kNormalise) {
                 // L = lost + c_i + c_j - X_ij (the point (i, i) receives its counter once); V~ = V * T / (T - L)
                 const int32_t x_ii = np.x[(long long)f * P + pair_index(n_inputs, i, i)];
-                const int32_t lost_ij = lost_f + x_ii + ((i != j) ? (x_jj - np.x[p]) : 0);
+                int32_t x_ij = 0;
+                if (i != j) {
+                    x_ij = np.x[p];
+                    if (x_ij) np.x[p] = 0;             // ends the integration: this thread is the only reader of X[p]
+                }
+                const int32_t lost_ij = lost_f + x_ii + ((i != j) ? (x_jj - x_ij) : 0);
                 const int32_t valid = (int32_t)np.n_samples - lost_ij;
                 const float scale = (valid > 0) ? __fdiv_rn((float)np.n_samples, (float)valid) : 0.0f;
                 *reinterpret_cast<float2 *>(reinterpret_cast<float *>(out_v) + p * 2) =
@@ -127,6 +132,15 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
             }
         }
     }
+}
+
+// after finalize_kernel<true>: flag counters (the diagonal of X) back to zero.  One thread per (f, input).
+__global__ void __launch_bounds__(256) clear_diag_kernel(int32_t *__restrict__ x, int n_inputs, int n_freq)
+{
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= (long long)n_inputs * n_freq) return;
+    const int f = (int)(k / n_inputs), n = (int)(k % n_inputs);
+    x[(long long)f * ((long long)n_inputs * (n_inputs + 1) / 2) + pair_index(n_inputs, n, n)] = 0;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -51,13 +51,15 @@ struct xcorr_handle {
     // lost-sample normalisation (xcorr_norm_enable): flag-intersection accumulator, packet-loss counters
     bool norm = false;
     int32_t *flag_x = nullptr;       // device int32[F][P]
-    int32_t *lost_dev = nullptr;     // device int32[F]
     int32_t *lost_dev_acc = nullptr; // device int32[F]: counters added on the device (xcorr_norm_process_dev)
     bool lost_dev_dirty = false;
-    int32_t *lost_pinned = nullptr;  // page-locked int32[F]: snapshot handed to the H2D copy of a read
+    int32_t *lost_dev = nullptr;     // device int32[F]: this integration's counters as finalize_kernel<true> reads them
+    int32_t *lost_pinned = nullptr;  // page-locked, device-mapped int32[2][F]: snapshots of lost_acc that lost_gather_kernel
+                                     // reads in place (no copy-engine operation in the stream); read r uses half r % 2
+    unsigned long long norm_reads = 0;
     long long *lost_acc = nullptr;   // host: lost samples per channel since the last read
     int32_t *staging_lost = nullptr; // device int32[F][P] for host reads of the normalisation matrix
-    cudaEvent_t lost_copied = nullptr;
+    cudaEvent_t lost_used[2] = {nullptr, nullptr};   // recorded after the finalize launch that read the snapshot half
     bool flags_dirty = false;        // flag_x holds counts of the current integration
 };
 
@@ -119,11 +121,12 @@ extern "C" void xcorr_destroy(xcorr_handle *h)
     cudaFree(h->worker_begin);
     cudaFree(h->tile_slot_begin);
     cudaFree(h->flag_x);
-    cudaFree(h->lost_dev);
     cudaFree(h->lost_dev_acc);
+    cudaFree(h->lost_dev);
     cudaFree(h->staging_lost);
     if (h->lost_pinned) cudaFreeHost(h->lost_pinned);
-    if (h->lost_copied) cudaEventDestroy(h->lost_copied);
+    for (int k = 0; k < 2; ++k)
+        if (h->lost_used[k]) cudaEventDestroy(h->lost_used[k]);
     delete[] h->lost_acc;
     delete h;
 }
@@ -295,15 +298,22 @@ static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *
         XC_CUDA(h, cudaMemsetAsync(h->sums, 0, h->sums_bytes, s));
     }
     NormParams np = {};
+    int lost_half = 0;
     if (normalise) {
-        // packet-loss counters: host accumulator -> page-locked snapshot -> device (the previous read's copy has long finished)
-        XC_CUDA(h, cudaEventSynchronize(h->lost_copied));
-        for (int f = 0; f < h->n_freq; ++f) h->lost_pinned[f] = (int32_t)h->lost_acc[f];
-        XC_CUDA(h, cudaMemcpyAsync(h->lost_dev, h->lost_pinned, sizeof(int32_t) * h->n_freq, cudaMemcpyHostToDevice, s));
-        XC_CUDA(h, cudaEventRecord(h->lost_copied, s));
-        np.x = h->flag_x;
+        // packet-loss counters: host accumulator -> page-locked snapshot the kernel reads in place; a half is reused two
+        // reads later, after the event recorded behind its reader
+        lost_half = (int)(h->norm_reads++ & 1u);
+        XC_CUDA(h, cudaEventSynchronize(h->lost_used[lost_half]));
+        int32_t *snap = h->lost_pinned + (size_t)lost_half * h->n_freq;
+        for (int f = 0; f < h->n_freq; ++f) snap[f] = (int32_t)h->lost_acc[f];
+        // lost_dev = host-counted snapshot + device-counted counters (xcorr_norm_process_dev), the latter cleared for the next integration
+        lost_gather_kernel<<<(h->n_freq + 255) / 256, 256, 0, s>>>(snap, h->lost_dev_acc, h->lost_dev, h->n_freq);
+        XC_CUDA(h, cudaGetLastError());
+        h->launches += 1;
+        XC_CUDA(h, cudaEventRecord(h->lost_used[lost_half], s));
+        h->lost_dev_dirty = false;
         np.lost = h->lost_dev;
-        np.lost_extra = h->lost_dev_acc;
+        np.x = h->flag_x;
         np.lost_out = lost_dst;
         np.n_samples = (uint32_t)h->samples_since_read;
     }
@@ -331,7 +341,16 @@ static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *
     h->offset_samples = 0;
     h->clean = true;
     if (h->norm) {   // the flag / loss state belongs to the integration that just ended
-        if (h->flags_dirty) XC_CUDA(h, cudaMemsetAsync(h->flag_x, 0, lost_matrix_bytes, s));
+        if (h->flags_dirty) {
+            if (normalise) {   // finalize_kernel<true> has already cleared the intersections it read; the counters remain
+                const long long nd = (long long)h->n_inputs * h->n_freq;
+                clear_diag_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, s>>>(h->flag_x, h->n_inputs, h->n_freq);
+                XC_CUDA(h, cudaGetLastError());
+                h->launches += 1;
+            } else {
+                XC_CUDA(h, cudaMemsetAsync(h->flag_x, 0, lost_matrix_bytes, s));
+            }
+        }
         h->flags_dirty = false;
         if (h->lost_dev_dirty) XC_CUDA(h, cudaMemsetAsync(h->lost_dev_acc, 0, sizeof(int32_t) * h->n_freq, s));
         h->lost_dev_dirty = false;
@@ -364,12 +383,11 @@ extern "C" int xcorr_norm_enable(xcorr_handle *h)
     if ((e = cudaMalloc(&h->staging_lost, lost_matrix_bytes)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
     if ((e = cudaMalloc(&h->lost_dev, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
     if ((e = cudaMalloc(&h->lost_dev_acc, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
-    if ((e = cudaMallocHost(&h->lost_pinned, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
+    if ((e = cudaMallocHost(&h->lost_pinned, sizeof(int32_t) * 2 * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
     h->lost_acc = new (std::nothrow) long long[h->n_freq]();
     if (!h->lost_acc) return XCORR_ENOMEM;
-    XC_CUDA(h, cudaEventCreateWithFlags(&h->lost_copied, cudaEventDisableTiming));
+    for (int k = 0; k < 2; ++k) XC_CUDA(h, cudaEventCreateWithFlags(&h->lost_used[k], cudaEventDisableTiming));
     XC_CUDA(h, cudaMemset(h->flag_x, 0, lost_matrix_bytes));
-    XC_CUDA(h, cudaMemset(h->lost_dev, 0, sizeof(int32_t) * h->n_freq));
     XC_CUDA(h, cudaMemset(h->lost_dev_acc, 0, sizeof(int32_t) * h->n_freq));
     h->norm = true;
     return XCORR_OK;
@@ -406,9 +424,9 @@ static int launch_flag_count(xcorr_handle *h, const uint8_t *flags_dev, void *cu
 {
     if (flags_dev) {
         const unsigned long long n_bytes = (unsigned long long)h->frame_bytes / 8;
-        const unsigned long long n_chunks = (n_bytes + 15) / 16;
-        int blocks = h->n_sms * 8;     // grid-stride, 8 resident CTAs of 256 threads per SM
-        if ((unsigned long long)blocks * 256ull > n_chunks) blocks = (int)((n_chunks + 255) / 256);
+        const unsigned long long n_pieces = (n_bytes + 16ull * 32 * kFlagUnroll - 1) / (16ull * 32 * kFlagUnroll);   // 2 KiB per warp and iteration
+        int blocks = h->n_sms * 8;     // warp-stride, 8 resident CTAs of 256 threads (8 warps) per SM
+        if ((unsigned long long)blocks * 8ull > n_pieces) blocks = (int)((n_pieces + 7) / 8);
         flag_count_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>(flags_dev, n_bytes, h->n_inputs, h->n_freq, h->flag_x);
         XC_CUDA(h, cudaGetLastError());
         h->launches += 1;

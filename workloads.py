@@ -249,3 +249,13 @@ def disturb_packets(packets: np.ndarray, seed: int, p_loss: float = 2e-3, p_dup:
         pos = np.sort(rng.integers(0, arrived.shape[0] + 1, n_foreign))
         arrived = np.insert(arrived, pos, extra, axis=0)
     return np.ascontiguousarray(arrived)
+
+
+def sparse_flag_bits(n_inputs: int, n_freq: int, n_time: int, seed: int, rate: float = 1e-4) -> np.ndarray:
+    """Cheap flag bit-field uint8[T][F][N/8] for full-size runs: about `rate` of the bytes get a random non-zero value
+    (1-8 inputs of one sample flagged together, E << N)."""
+    rng = np.random.default_rng(seed)
+    fb = np.zeros((n_time, n_freq, n_inputs // 8), dtype=np.uint8)
+    hit = rng.integers(0, fb.size, max(1, int(fb.size * rate)))
+    fb.reshape(-1)[hit] = rng.integers(1, 256, hit.size, dtype=np.uint8)
+    return fb
