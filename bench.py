@@ -35,7 +35,7 @@ import workloads as wl  # noqa: E402
 NOMINAL_INT8_TOPS = 4500.0  # dense int8, B200 nominal (2x the 2.25 PFLOP/s dense bf16 figure)
 # dram__bytes_read.sum + dram__bytes_write.sum of xengine_kernel<false> for one C2 launch, from the committed
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = {"C2": 292.3e6}   # profiles/r01_ncu_full_bench_c2.md: 268.49 MB read + 23.77 MB written
+NCU_TRAFFIC_BYTES = {"C2": 277.7e6}   # profiles/r01_ncu_full_bench_c2.md: 268.49 MB read + 9.17 MB written
 
 
 def load_peaks():
@@ -133,6 +133,10 @@ def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
     ev = lambda: torch.cuda.Event(enable_timing=True)
     names = ["assemble", "process", "norm_process", "read_normalized"]
     times = {k: [] for k in names}
+    for _ in range(200):                         # the host-side packet generation let the clocks drop: bring them back up
+        x.process(frame, st)
+        x.read(vis.view(torch.int32), st)
+    evs = []
     for r in range(reps + 3):
         e = [ev() for _ in range(5)]
         with torch.cuda.stream(st):
@@ -145,10 +149,11 @@ def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
             e[3].record(st)
             x.read_normalized(vis, stream=st)
             e[4].record(st)
-        torch.cuda.synchronize()
-        if r >= 3:
-            for k, nm in enumerate(names):
-                times[nm].append(e[k].elapsed_time(e[k + 1]) * 1e3)
+        evs.append(e)
+    torch.cuda.synchronize()
+    for e in evs[3:]:
+        for k, nm in enumerate(names):
+            times[nm].append(e[k].elapsed_time(e[k + 1]) * 1e3)
     c = counts.cpu().tolist()
     a.close()
     us = {k: statistics.mean(v) for k, v in times.items()}
@@ -160,7 +165,7 @@ def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
         "packets": n_pk, "packet_bytes": pbytes, "kept_dup_rejected_lostpos": c, "us": us,
         "assemble_roofline": {"bound": "hbm", "achieved": asm_bytes / (us["assemble"] * 1e-6) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                               "frac": asm_bytes / (us["assemble"] * 1e-6) / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": asm_bytes,
-                              "note": "2 kernels (packet_claim_kernel + assemble_kernel) and 3 small memsets in the timed call"},
+                              "note": "2 kernels in the timed call: packet_claim_kernel + assemble_kernel"},
         "flag_count_roofline": {"bound": "hbm", "achieved": flag_bytes / (us["norm_process"] * 1e-6) / 1e9, "peak": peaks["hbm_gbs"],
                                 "unit": "GB/s", "frac": flag_bytes / (us["norm_process"] * 1e-6) / 1e9 / peaks["hbm_gbs"],
                                 "algorithmic_bytes": flag_bytes,

@@ -35,11 +35,14 @@ struct AssembleShape {
 };
 
 // counts[0] kept  [1] duplicates  [2] rejected  [3] positions lost  [4] valid (scratch)  [5] CTA ticket (scratch)
+// The ownership table and the counters are all-kNoOwner / all-zero on entry: xcorr_assembler_create leaves them so, and
+// assemble_kernel puts every word it consumed back (no memset between calls).  `lost` (caller's int32[F]) is zeroed here.
 __global__ void __launch_bounds__(256) packet_claim_kernel(const uint8_t *__restrict__ packets, unsigned int n_packets,
                                                             unsigned long long seq0, AssembleShape sh, uint32_t *__restrict__ owner,
-                                                            uint32_t *__restrict__ counts)
+                                                            uint32_t *__restrict__ counts, int32_t *__restrict__ lost)
 {
     const unsigned int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (lost && k < (unsigned)sh.n_freq) lost[k] = 0;
     bool valid = false, rejected = false;
     if (k < n_packets) {
         const uint4 hdr = __ldg(reinterpret_cast<const uint4 *>(packets + (unsigned long long)k * sh.packet_bytes));
@@ -63,8 +66,9 @@ __global__ void __launch_bounds__(256) packet_claim_kernel(const uint8_t *__rest
 __device__ __forceinline__ uint32_t spread4(uint32_t x) { return (((x & 0xFu) * 0x00204081u) & 0x01010101u) * 0xFFu; }
 
 __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict__ packets, AssembleShape sh,
-                                                        const uint32_t *__restrict__ owner, uint8_t *__restrict__ frame,
-                                                        uint8_t *__restrict__ flags, int32_t *__restrict__ lost, uint32_t *__restrict__ counts)
+                                                        uint32_t *__restrict__ owner, uint8_t *__restrict__ frame,
+                                                        uint8_t *__restrict__ flags, int32_t *__restrict__ lost, uint32_t *__restrict__ counts,
+                                                        uint32_t *__restrict__ counts_out)
 {
     const int N = sh.n_inputs, F = sh.n_freq, S = sh.s_per_packet, C = sh.c_per_packet;
     const unsigned row_chunks = (unsigned)(C * N) >> 4;            // 16-byte vectors per time sample of one stream
@@ -76,7 +80,9 @@ __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict
     uint32_t kept_local = 0, lost_local = 0;                      // thread 0's tallies of this CTA
     for (unsigned pos = blockIdx.x; pos < n_pos; pos += gridDim.x) {
         const unsigned blk = pos / (unsigned)sh.n_streams, stream = pos % (unsigned)sh.n_streams;
-        const uint32_t own = __ldg(owner + pos);
+        const uint32_t own = owner[pos];                           // this CTA is the position's only reader:
+        __syncthreads();
+        if (threadIdx.x == 0 && own != kNoOwner) owner[pos] = kNoOwner;   // ... and leaves the table clean for the next frame
         // byte offset of (t = blk*S, f = C*stream, n = 0) in the frame; rows of one stream are C*N contiguous bytes, F*N apart
         const unsigned long long f0 = ((unsigned long long)blk * S * F + (unsigned long long)C * stream) * (unsigned long long)N;
         uint4 *frame_v = reinterpret_cast<uint4 *>(frame + f0);
@@ -124,15 +130,20 @@ __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict
             lost_local += 1;
         }
     }
-    // packet counts: one atomic per CTA; the last CTA to finish derives duplicates = valid - kept
-    if (counts && threadIdx.x == 0) {
+    // packet counts: one atomic per CTA; the last CTA to finish derives duplicates = valid - kept, hands the four
+    // numbers to the caller and zeroes the scratch for the next frame
+    if (threadIdx.x == 0) {
         if (kept_local) atomicAdd(counts + 0, kept_local);
         if (lost_local) atomicAdd(counts + 3, lost_local);
         __threadfence();
         if (atomicAdd(counts + 5, 1u) == gridDim.x - 1) {
             __threadfence();
-            const uint32_t kept = atomicAdd(counts + 0, 0u), valid = atomicAdd(counts + 4, 0u);
-            counts[1] = valid - kept;
+            const uint32_t kept = atomicExch(counts + 0, 0u), valid = atomicExch(counts + 4, 0u);
+            const uint32_t rejected = atomicExch(counts + 2, 0u), lost_pos = atomicExch(counts + 3, 0u);
+            counts[5] = 0;
+            if (counts_out) {
+                counts_out[0] = kept; counts_out[1] = valid - kept; counts_out[2] = rejected; counts_out[3] = lost_pos;
+            }
         }
     }
 }

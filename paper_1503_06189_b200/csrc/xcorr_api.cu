@@ -624,6 +624,11 @@ extern "C" int xcorr_assembler_create(int n_inputs, int n_freq, int t_per_frame,
         xcorr_assembler_destroy(a);
         return e == cudaErrorMemoryAllocation ? XCORR_ENOMEM : XCORR_ECUDA;
     }
+    if ((e = cudaMemset(a->owner, 0xFF, sizeof(uint32_t) * (size_t)a->n_positions)) != cudaSuccess ||
+        (e = cudaMemset(a->counts, 0, sizeof(uint32_t) * 8)) != cudaSuccess) {
+        xcorr_assembler_destroy(a);
+        return XCORR_ECUDA;
+    }
     *out = a;
     return XCORR_OK;
 }
@@ -636,21 +641,20 @@ extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_
         ((uintptr_t)counts_dev & 3u))
         return XCORR_EINVAL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    XC_CUDA(a, cudaMemsetAsync(a->owner, 0xFF, sizeof(uint32_t) * (size_t)a->n_positions, s));
-    XC_CUDA(a, cudaMemsetAsync(a->counts, 0, sizeof(uint32_t) * 8, s));
-    if (lost_dev) XC_CUDA(a, cudaMemsetAsync(lost_dev, 0, sizeof(int32_t) * a->sh.n_freq, s));
-    if (n_packets) {
-        packet_claim_kernel<<<(unsigned)((n_packets + 255) / 256), 256, 0, s>>>((const uint8_t *)packets, (unsigned)n_packets, seq0, a->sh,
-                                                                               a->owner, a->counts);
+    // no memsets: the ownership table and counters are left clean by the previous call's assemble_kernel (see create)
+    {
+        size_t n_threads = n_packets > (size_t)a->sh.n_freq ? n_packets : (size_t)a->sh.n_freq;   // also zeroes lost_dev[F]
+        packet_claim_kernel<<<(unsigned)((n_threads + 255) / 256), 256, 0, s>>>((const uint8_t *)packets, (unsigned)n_packets, seq0, a->sh,
+                                                                               a->owner, a->counts, lost_dev);
         XC_CUDA(a, cudaGetLastError());
         a->launches += 1;
     }
     // grid-stride over the positions: 8 resident CTAs of 256 threads per SM
     unsigned blocks = (unsigned)a->n_sms * 8u;
     if (blocks > a->n_positions) blocks = a->n_positions;
-    assemble_kernel<<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, a->owner, (uint8_t *)frame_dev, flags_dev, lost_dev, a->counts);
+    assemble_kernel<<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, a->owner, (uint8_t *)frame_dev, flags_dev, lost_dev, a->counts,
+                                           counts_dev);
     XC_CUDA(a, cudaGetLastError());
     a->launches += 1;
-    if (counts_dev) XC_CUDA(a, cudaMemcpyAsync(counts_dev, a->counts, sizeof(uint32_t) * 4, cudaMemcpyDefault, s));
     return XCORR_OK;
 }
