@@ -201,6 +201,15 @@ int xcorr_stream_sync(xcorr_stream *s);
  */
 int xcorr_stream_read(xcorr_stream *s, int32_t *upper_triangle_out);
 
+/*
+ * xcorr_stream_read_async -- the same read enqueued on the compute stream WITHOUT waiting: the call returns at once,
+ * the next xcorr_stream_submit() may follow immediately (its host-to-device copy then overlaps this read's kernel
+ * and device-to-host copy -- PCIe is full duplex), and `upper_triangle_out` (host, page-locked for the overlap, or
+ * device) holds the result once xcorr_stream_sync() has returned.  BORROWED until then.  Ends the integration like
+ * xcorr_read(): frames submitted afterwards belong to the next one.
+ */
+int xcorr_stream_read_async(xcorr_stream *s, int32_t *upper_triangle_out);
+
 /* Release buffers, streams and events (synchronises first).  NULL is a no-op. */
 void xcorr_stream_destroy(xcorr_stream *s);
 

@@ -17,7 +17,7 @@ __all__ = [
     "XCorrError", "lib", "xcorr_create", "xcorr_process", "xcorr_read", "xcorr_destroy", "xcorr_strerror",
     "xcorr_last_cuda_error", "xcorr_frame_bytes", "xcorr_output_bytes", "xcorr_kernel_launches",
     "xcorr_norm_enable", "xcorr_norm_process", "xcorr_read_normalized",
-    "xcorr_stream_create", "xcorr_stream_submit", "xcorr_stream_sync", "xcorr_stream_read", "xcorr_stream_destroy",
+    "xcorr_stream_create", "xcorr_stream_submit", "xcorr_stream_sync", "xcorr_stream_read", "xcorr_stream_read_async", "xcorr_stream_destroy",
     "xcorr_assembler_create", "xcorr_assembler_packet_bytes", "xcorr_assemble", "xcorr_assembler_kernel_launches",
     "xcorr_assembler_destroy", "xcorr_norm_process_dev",
     "xcorr_debug_schedule", "xcorr_debug_stage_samples", "xcorr_debug_process_simt", "XCorr", "XCorrStream", "Assembler",
@@ -84,6 +84,8 @@ def lib() -> ctypes.CDLL:
     L.xcorr_stream_sync.restype = ci
     L.xcorr_stream_read.argtypes = [vp, vp]
     L.xcorr_stream_read.restype = ci
+    L.xcorr_stream_read_async.argtypes = [vp, vp]
+    L.xcorr_stream_read_async.restype = ci
     L.xcorr_stream_destroy.argtypes = [vp]
     L.xcorr_stream_destroy.restype = None
     L.xcorr_assembler_create.argtypes = [ci, ci, ci, ci, ci, ctypes.POINTER(vp)]
@@ -206,6 +208,10 @@ def xcorr_stream_sync(stream: int) -> int:
 
 def xcorr_stream_read(stream: int, upper_triangle_out: int) -> int:
     return lib().xcorr_stream_read(stream, upper_triangle_out)
+
+
+def xcorr_stream_read_async(stream: int, upper_triangle_out: int) -> int:
+    return lib().xcorr_stream_read_async(stream, upper_triangle_out)
 
 
 def xcorr_stream_destroy(stream: int) -> None:
@@ -373,6 +379,12 @@ class XCorrStream:
     def read(self, out):
         ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
         self.xc._check(xcorr_stream_read(self.stream, ptr), "xcorr_stream_read")
+        return out
+
+    def read_async(self, out):
+        """Enqueue the read without waiting; ``out`` is valid after ``sync()``."""
+        ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        self.xc._check(xcorr_stream_read_async(self.stream, ptr), "xcorr_stream_read_async")
         return out
 
     def close(self) -> None:

@@ -283,7 +283,7 @@ static bool is_device_pointer(const void *ptr)
 }
 
 // xcorr_read / xcorr_read_normalized: one launch of finalize_kernel; ends the integration
-static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *lost_matrix_out, void *cuda_stream)
+static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *lost_matrix_out, void *cuda_stream, bool wait = true)
 {
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const bool on_device = is_device_pointer(vis_out);
@@ -359,7 +359,7 @@ static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *
     if (!on_device) XC_CUDA(h, cudaMemcpyAsync(vis_out, h->staging, h->output_bytes, cudaMemcpyDeviceToHost, s));
     if (lost_matrix_out && !lost_on_device)
         XC_CUDA(h, cudaMemcpyAsync(lost_matrix_out, h->staging_lost, lost_matrix_bytes, cudaMemcpyDeviceToHost, s));
-    if (!on_device || (lost_matrix_out && !lost_on_device)) XC_CUDA(h, cudaStreamSynchronize(s));
+    if (wait && (!on_device || (lost_matrix_out && !lost_on_device))) XC_CUDA(h, cudaStreamSynchronize(s));
     return XCORR_OK;
 }
 
@@ -515,6 +515,12 @@ extern "C" int xcorr_stream_read(xcorr_stream *s, int32_t *upper_triangle_out)
     if (rc != XCORR_OK) return rc;
     XC_CUDA(s->h, cudaStreamSynchronize(s->compute_stream));
     return XCORR_OK;
+}
+
+extern "C" int xcorr_stream_read_async(xcorr_stream *s, int32_t *upper_triangle_out)
+{
+    if (!s || !upper_triangle_out) return XCORR_EINVAL;
+    return read_common(s->h, upper_triangle_out, false, nullptr, (void *)s->compute_stream, /*wait=*/false);
 }
 
 // ---------------------------------------------------------------------------------------------------

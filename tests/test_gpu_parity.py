@@ -184,6 +184,14 @@ def test_streamed_path_matches_oracle(xb):
     dout = torch.empty((f, x.n_pairs, 2), dtype=torch.int32, device="cuda")
     s.read(dout)
     assert np.array_equal(dout.cpu().numpy(), oracle.planar(frames[0]).astype(np.int64) + oracle.planar(frames[1]))
+    # asynchronous reads: one integration per frame, the next submit follows at once, results valid after sync()
+    outs = [torch.empty((f, x.n_pairs, 2), dtype=torch.int32).pin_memory() for _ in frames]
+    for p, o in zip(pinned, outs):
+        s.submit(p)
+        s.read_async(o)
+    s.sync()
+    for fr, o in zip(frames, outs):
+        assert np.array_equal(o.numpy(), oracle.planar(fr))
     s.close()
     x.close()
 
