@@ -35,8 +35,9 @@ struct AssembleShape {
 };
 
 // counts[0] kept  [1] duplicates  [2] rejected  [3] positions lost  [4] valid (scratch)  [5] CTA ticket (scratch)
-// The ownership table and the counters are all-kNoOwner / all-zero on entry: xcorr_assembler_create leaves them so, and
-// assemble_kernel puts every word it consumed back (no memset between calls).  `lost` (caller's int32[F]) is zeroed here.
+// The ownership table and the counters are all-kNoOwner / all-zero on entry (no memset between calls): there are two
+// tables used alternately, assemble_kernel resets the one the previous frame used while it reads this frame's, and its
+// last CTA zeroes the counters.  `lost` (caller's int32[F]) is zeroed here.
 __global__ void __launch_bounds__(256) packet_claim_kernel(const uint8_t *__restrict__ packets, unsigned int n_packets,
                                                             unsigned long long seq0, AssembleShape sh, uint32_t *__restrict__ owner,
                                                             uint32_t *__restrict__ counts, int32_t *__restrict__ lost)
@@ -66,7 +67,8 @@ __global__ void __launch_bounds__(256) packet_claim_kernel(const uint8_t *__rest
 __device__ __forceinline__ uint32_t spread4(uint32_t x) { return (((x & 0xFu) * 0x00204081u) & 0x01010101u) * 0xFFu; }
 
 __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict__ packets, AssembleShape sh,
-                                                        uint32_t *__restrict__ owner, uint8_t *__restrict__ frame,
+                                                        const uint32_t *__restrict__ owner, uint32_t *__restrict__ owner_next,
+                                                        uint8_t *__restrict__ frame,
                                                         uint8_t *__restrict__ flags, int32_t *__restrict__ lost, uint32_t *__restrict__ counts,
                                                         uint32_t *__restrict__ counts_out)
 {
@@ -80,9 +82,8 @@ __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict
     uint32_t kept_local = 0, lost_local = 0;                      // thread 0's tallies of this CTA
     for (unsigned pos = blockIdx.x; pos < n_pos; pos += gridDim.x) {
         const unsigned blk = pos / (unsigned)sh.n_streams, stream = pos % (unsigned)sh.n_streams;
-        const uint32_t own = owner[pos];                           // this CTA is the position's only reader:
-        __syncthreads();
-        if (threadIdx.x == 0 && own != kNoOwner) owner[pos] = kNoOwner;   // ... and leaves the table clean for the next frame
+        const uint32_t own = __ldg(owner + pos);
+        if (threadIdx.x == 0) owner_next[pos] = kNoOwner;          // the table the NEXT frame's claims go to (last frame's, dirty)
         // byte offset of (t = blk*S, f = C*stream, n = 0) in the frame; rows of one stream are C*N contiguous bytes, F*N apart
         const unsigned long long f0 = ((unsigned long long)blk * S * F + (unsigned long long)C * stream) * (unsigned long long)N;
         uint4 *frame_v = reinterpret_cast<uint4 *>(frame + f0);
@@ -91,17 +92,29 @@ __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict
             const uint8_t *pkt = packets + (unsigned long long)own * sh.packet_bytes;
             const uint4 *pay = reinterpret_cast<const uint4 *>(pkt + kPacketHeaderBytes);
             const uint16_t *foot16 = reinterpret_cast<const uint16_t *>(pkt + kPacketHeaderBytes + pay_bytes);
-            for (unsigned c = threadIdx.x; c < pay_chunks; c += blockDim.x) {
-                uint4 v = __ldg(pay + c);
-                const uint32_t bits = __ldg(foot16 + c);           // the 16 flag bits of these 16 inputs
-                if (bits) {                                        // rare: zero the flagged samples' bytes (P5)
-                    v.x &= ~spread4(bits);
-                    v.y &= ~spread4(bits >> 4);
-                    v.z &= ~spread4(bits >> 8);
-                    v.w &= ~spread4(bits >> 12);
+            // two vectors per thread in flight (both loads issued before the first store)
+            for (unsigned c0 = threadIdx.x; c0 < pay_chunks; c0 += 2 * blockDim.x) {
+                const unsigned c1 = c0 + blockDim.x;
+                const bool two = c1 < pay_chunks;
+                uint4 v0 = __ldg(pay + c0), v1 = make_uint4(0, 0, 0, 0);
+                const uint32_t bits0 = __ldg(foot16 + c0);         // the 16 flag bits of these 16 inputs
+                uint32_t bits1 = 0;
+                if (two) {
+                    v1 = __ldg(pay + c1);
+                    bits1 = __ldg(foot16 + c1);
                 }
-                const unsigned dt = c / row_chunks, w = c - dt * row_chunks;
-                frame_v[dt * frame_row_stride + w] = v;
+                if (bits0 | bits1) {                               // rare: zero the flagged samples' bytes (P5)
+                    v0.x &= ~spread4(bits0);       v0.y &= ~spread4(bits0 >> 4);
+                    v0.z &= ~spread4(bits0 >> 8);  v0.w &= ~spread4(bits0 >> 12);
+                    v1.x &= ~spread4(bits1);       v1.y &= ~spread4(bits1 >> 4);
+                    v1.z &= ~spread4(bits1 >> 8);  v1.w &= ~spread4(bits1 >> 12);
+                }
+                const unsigned dt0 = c0 / row_chunks, w0 = c0 - dt0 * row_chunks;
+                frame_v[dt0 * frame_row_stride + w0] = v0;
+                if (two) {
+                    const unsigned dt1 = c1 / row_chunks, w1 = c1 - dt1 * row_chunks;
+                    frame_v[dt1 * frame_row_stride + w1] = v1;
+                }
             }
             if (flags) {
                 const uint4 *foot = reinterpret_cast<const uint4 *>(foot16);

@@ -579,7 +579,9 @@ struct xcorr_assembler {
     AssembleShape sh = {};
     int device = 0, n_sms = 0;
     unsigned n_positions = 0;
-    uint32_t *owner = nullptr;     // device uint32[n_positions]: arrival index of the packet that owns the position
+    uint32_t *owner = nullptr;     // device uint32[2][n_positions]: arrival index of the packet that owns the position; the
+                                   // two tables alternate from call to call (assemble_kernel.cuh)
+    unsigned long long calls = 0;
     uint32_t *counts = nullptr;    // device uint32[8], see assemble_kernel.cuh
     uint64_t launches = 0;
     int last_cuda_error = 0;
@@ -624,13 +626,13 @@ extern "C" int xcorr_assembler_create(int n_inputs, int n_freq, int t_per_frame,
     a->sh.packet_bytes = kPacketHeaderBytes + pay + pay / 8;
     a->n_positions = (unsigned)a->sh.n_streams * (unsigned)a->sh.n_blocks;
     cudaError_t e;
-    if ((e = cudaMalloc(&a->owner, sizeof(uint32_t) * (size_t)a->n_positions)) != cudaSuccess ||
+    if ((e = cudaMalloc(&a->owner, sizeof(uint32_t) * 2 * (size_t)a->n_positions)) != cudaSuccess ||
         (e = cudaMalloc(&a->counts, sizeof(uint32_t) * 8)) != cudaSuccess) {
         cudaGetLastError();
         xcorr_assembler_destroy(a);
         return e == cudaErrorMemoryAllocation ? XCORR_ENOMEM : XCORR_ECUDA;
     }
-    if ((e = cudaMemset(a->owner, 0xFF, sizeof(uint32_t) * (size_t)a->n_positions)) != cudaSuccess ||
+    if ((e = cudaMemset(a->owner, 0xFF, sizeof(uint32_t) * 2 * (size_t)a->n_positions)) != cudaSuccess ||
         (e = cudaMemset(a->counts, 0, sizeof(uint32_t) * 8)) != cudaSuccess) {
         xcorr_assembler_destroy(a);
         return XCORR_ECUDA;
@@ -647,19 +649,22 @@ extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_
         ((uintptr_t)counts_dev & 3u))
         return XCORR_EINVAL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    // no memsets: the ownership table and counters are left clean by the previous call's assemble_kernel (see create)
+    // no memsets: the ownership tables and counters are left clean by the previous call's assemble_kernel (see create)
+    uint32_t *owner = a->owner + (size_t)(a->calls & 1u) * a->n_positions;
+    uint32_t *owner_next = a->owner + (size_t)((a->calls + 1) & 1u) * a->n_positions;
+    a->calls += 1;
     {
         size_t n_threads = n_packets > (size_t)a->sh.n_freq ? n_packets : (size_t)a->sh.n_freq;   // also zeroes lost_dev[F]
         packet_claim_kernel<<<(unsigned)((n_threads + 255) / 256), 256, 0, s>>>((const uint8_t *)packets, (unsigned)n_packets, seq0, a->sh,
-                                                                               a->owner, a->counts, lost_dev);
+                                                                               owner, a->counts, lost_dev);
         XC_CUDA(a, cudaGetLastError());
         a->launches += 1;
     }
     // grid-stride over the positions: 8 resident CTAs of 256 threads per SM
     unsigned blocks = (unsigned)a->n_sms * 8u;
     if (blocks > a->n_positions) blocks = a->n_positions;
-    assemble_kernel<<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, a->owner, (uint8_t *)frame_dev, flags_dev, lost_dev, a->counts,
-                                           counts_dev);
+    assemble_kernel<<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, owner, owner_next, (uint8_t *)frame_dev, flags_dev, lost_dev,
+                                           a->counts, counts_dev);
     XC_CUDA(a, cudaGetLastError());
     a->launches += 1;
     return XCORR_OK;
