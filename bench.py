@@ -155,6 +155,24 @@ def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
         for k, nm in enumerate(names):
             times[nm].append(e[k].elapsed_time(e[k + 1]) * 1e3)
     c = counts.cpu().tolist()
+    # the same chain end to end from page-locked HOST packet rings: xcorr_stream_submit_packets per frame (H2D copy of the
+    # ring, assemble, correlate, flag / loss accounting) and one normalised read into host memory per frame
+    pk_host = [p.cpu().pin_memory() for p in pk_dev]
+    del pk_dev
+    xs = xb.XCorrStream(x, depth=2)
+    xs.attach_assembler(a, n_pk)
+    vis_host = torch.empty((f, cfg.n_pairs, 2), dtype=torch.float32).pin_memory()
+    for k in range(2):
+        xs.submit_packets(pk_host[k % 2], n_pk, 10 ** 12)
+        xs.read_normalized(vis_host)
+    n_pe = 10
+    t0 = time.perf_counter()
+    for k in range(n_pe):
+        xs.submit_packets(pk_host[k % 2], n_pk, 10 ** 12)
+        xs.read_normalized(vis_host)
+    torch.cuda.synchronize()
+    dt_pe = time.perf_counter() - t0
+    xs.close()
     a.close()
     us = {k: statistics.mean(v) for k, v in times.items()}
     asm_bytes = n_pk * pbytes + cfg.frame_bytes + cfg.frame_bytes // 8
@@ -171,6 +189,9 @@ def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
                                 "algorithmic_bytes": flag_bytes,
                                 "note": "flag_count_kernel + lost_add_kernel; the flag field was just written, so part of it is an L2 hit"},
         "pipeline_gbps": 8.0 * cfg.frame_bytes / (sum(us.values()) * 1e-6) / 1e9,
+        "e2e_packets": {"value": 8.0 * cfg.frame_bytes * n_pe / dt_pe / 1e9, "unit": "Gb/s of frame (sky) data", "steps": n_pe,
+                        "ms_per_step": dt_pe / n_pe * 1e3, "h2d_bytes_per_step": n_pk * pbytes, "d2h_bytes_per_step": cfg.output_bytes,
+                        "api": "xcorr_stream_submit_packets(pinned host packet ring) + xcorr_stream_read_normalized(pinned host out)"},
     }
 
 

@@ -106,6 +106,32 @@ void xcorr_assembler_destroy(xcorr_assembler *a);
  */
 int xcorr_norm_process_dev(xcorr_handle *h, const uint8_t *flags_dev, const int32_t *lost_samples_dev, void *cuda_stream);
 
+/* ---------------------------------------------------------------------------------------------------
+ * Streamed packet path: what one server of the paper does per frame (Fig. 2, :47, :63) -- packets in a
+ * page-locked host ring -> copy to the GPU -> assemble -> correlate -> (flag / loss accounting) -- on the two
+ * streams of an xcorr_stream (xcorr.h, row a5), the copy of frame k+1's packets overlapping the kernels of frame k.
+ * ------------------------------------------------------------------------------------------------- */
+
+/*
+ * xcorr_stream_attach_assembler -- startup-time call: gives the stream's `depth` ring slots a device buffer for
+ * `max_packets` packets, a flag field and loss counters.  `a` (same N, F, T as the stream's handle) is BORROWED
+ * until the stream is destroyed.  Once per stream.  Errors: EINVAL, ENOMEM.
+ */
+int xcorr_stream_attach_assembler(xcorr_stream *s, xcorr_assembler *a, size_t max_packets);
+
+/*
+ * xcorr_stream_submit_packets -- enqueue one frame given as its packets in arrival order (page-locked host memory,
+ * n_packets <= max_packets, layout as for xcorr_assemble): H2D copy on the copy stream, then on the compute stream
+ * xcorr_assemble -> xcorr_process and, if the handle has normalisation enabled, xcorr_norm_process_dev with the
+ * frame's flag field and loss counters.  `packets_host` is BORROWED until the copy has completed (as in
+ * xcorr_stream_submit).  Returns without waiting unless all ring slots are in flight.
+ * Errors: EINVAL, EOVERFLOW, ECUDA.
+ */
+int xcorr_stream_submit_packets(xcorr_stream *s, const void *packets_host, size_t n_packets, uint64_t seq0);
+
+/* xcorr_read_normalized() ordered after all submitted frames on the compute stream; returns after the data has landed. */
+int xcorr_stream_read_normalized(xcorr_stream *s, float *vis_out, int32_t *lost_matrix_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,7 +19,8 @@ __all__ = [
     "xcorr_norm_enable", "xcorr_norm_process", "xcorr_read_normalized",
     "xcorr_stream_create", "xcorr_stream_submit", "xcorr_stream_sync", "xcorr_stream_read", "xcorr_stream_read_async", "xcorr_stream_destroy",
     "xcorr_assembler_create", "xcorr_assembler_packet_bytes", "xcorr_assemble", "xcorr_assembler_kernel_launches",
-    "xcorr_assembler_destroy", "xcorr_norm_process_dev",
+    "xcorr_assembler_destroy", "xcorr_norm_process_dev", "xcorr_stream_attach_assembler", "xcorr_stream_submit_packets",
+    "xcorr_stream_read_normalized",
     "xcorr_debug_schedule", "xcorr_debug_stage_samples", "xcorr_debug_process_simt", "XCorr", "XCorrStream", "Assembler",
 ]
 
@@ -100,6 +101,12 @@ def lib() -> ctypes.CDLL:
     L.xcorr_assembler_destroy.restype = None
     L.xcorr_norm_process_dev.argtypes = [vp, vp, vp, vp]
     L.xcorr_norm_process_dev.restype = ci
+    L.xcorr_stream_attach_assembler.argtypes = [vp, vp, ctypes.c_size_t]
+    L.xcorr_stream_attach_assembler.restype = ci
+    L.xcorr_stream_submit_packets.argtypes = [vp, vp, ctypes.c_size_t, ctypes.c_uint64]
+    L.xcorr_stream_submit_packets.restype = ci
+    L.xcorr_stream_read_normalized.argtypes = [vp, vp, vp]
+    L.xcorr_stream_read_normalized.restype = ci
     L.xcorr_debug_schedule.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ctypes.c_int32), ci, ctypes.POINTER(ctypes.c_int32)]
     L.xcorr_debug_schedule.restype = ci
     L.xcorr_debug_stage_samples.argtypes = []
@@ -212,6 +219,18 @@ def xcorr_stream_read(stream: int, upper_triangle_out: int) -> int:
 
 def xcorr_stream_read_async(stream: int, upper_triangle_out: int) -> int:
     return lib().xcorr_stream_read_async(stream, upper_triangle_out)
+
+
+def xcorr_stream_attach_assembler(stream: int, assembler: int, max_packets: int) -> int:
+    return lib().xcorr_stream_attach_assembler(stream, assembler, int(max_packets))
+
+
+def xcorr_stream_submit_packets(stream: int, packets_host: int, n_packets: int, seq0: int) -> int:
+    return lib().xcorr_stream_submit_packets(stream, packets_host or None, int(n_packets), int(seq0))
+
+
+def xcorr_stream_read_normalized(stream: int, vis_out: int, lost_matrix_out: int = 0) -> int:
+    return lib().xcorr_stream_read_normalized(stream, vis_out, lost_matrix_out or None)
 
 
 def xcorr_stream_destroy(stream: int) -> None:
@@ -379,6 +398,27 @@ class XCorrStream:
     def read(self, out):
         ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
         self.xc._check(xcorr_stream_read(self.stream, ptr), "xcorr_stream_read")
+        return out
+
+    def attach_assembler(self, assembler, max_packets: int) -> None:
+        """Packet path: ``assembler`` is an ``Assembler`` of the same shape; keeps a reference to it."""
+        self.xc._check(xcorr_stream_attach_assembler(self.stream, assembler.handle, max_packets), "xcorr_stream_attach_assembler")
+        self.assembler = assembler
+
+    def submit_packets(self, packets_host, n_packets: int, seq0: int) -> None:
+        """packets_host: contiguous (pinned) CPU uint8 tensor / numpy array holding n_packets packets in arrival order."""
+        if hasattr(packets_host, "data_ptr"):
+            ptr, nbytes = packets_host.data_ptr(), packets_host.numel() * packets_host.element_size()
+        else:
+            ptr, nbytes = packets_host.ctypes.data, packets_host.nbytes
+        if nbytes < n_packets * self.assembler.packet_bytes:
+            raise ValueError("packets_host holds fewer than n_packets packets")
+        self.xc._check(xcorr_stream_submit_packets(self.stream, ptr, n_packets, seq0), "xcorr_stream_submit_packets")
+
+    def read_normalized(self, out, lost_out=None):
+        lptr = 0 if lost_out is None else (lost_out.data_ptr() if hasattr(lost_out, "data_ptr") else lost_out.ctypes.data)
+        ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        self.xc._check(xcorr_stream_read_normalized(self.stream, ptr, lptr), "xcorr_stream_read_normalized")
         return out
 
     def read_async(self, out):

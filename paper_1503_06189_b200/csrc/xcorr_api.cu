@@ -70,6 +70,12 @@ struct xcorr_stream {
     cudaEvent_t copied[8] = {}, consumed[8] = {};
     cudaStream_t copy_stream = nullptr, compute_stream = nullptr;
     unsigned long long submitted = 0;
+    // packet path (xcorr_stream_attach_assembler): per ring slot a device copy of the packets, the flag field and the counters
+    struct xcorr_assembler *assembler = nullptr;   // borrowed
+    size_t max_packets = 0;
+    uint8_t *pkt_buf[8] = {};
+    uint8_t *flags_buf[8] = {};
+    int32_t *lost_buf[8] = {};
 };
 
 #define XC_CUDA(h, expr)                                  \
@@ -452,6 +458,9 @@ extern "C" void xcorr_stream_destroy(xcorr_stream *s)
     cudaDeviceSynchronize();
     for (int k = 0; k < s->depth; ++k) {
         if (s->buf[k]) cudaFree(s->buf[k]);
+        if (s->pkt_buf[k]) cudaFree(s->pkt_buf[k]);
+        if (s->flags_buf[k]) cudaFree(s->flags_buf[k]);
+        if (s->lost_buf[k]) cudaFree(s->lost_buf[k]);
         if (s->copied[k]) cudaEventDestroy(s->copied[k]);
         if (s->consumed[k]) cudaEventDestroy(s->consumed[k]);
     }
@@ -667,5 +676,61 @@ extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_
                                            a->counts, counts_dev);
     XC_CUDA(a, cudaGetLastError());
     a->launches += 1;
+    return XCORR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// streamed packet path: page-locked packet ring -> H2D -> assemble -> correlate (-> flag / loss accounting)
+// ---------------------------------------------------------------------------------------------------
+extern "C" int xcorr_stream_attach_assembler(xcorr_stream *s, xcorr_assembler *a, size_t max_packets)
+{
+    if (!s || !a || max_packets == 0 || max_packets > 0x7FFFFFFEull || s->assembler) return XCORR_EINVAL;
+    xcorr_handle *h = s->h;
+    if (a->sh.n_inputs != h->n_inputs || a->sh.n_freq != h->n_freq || a->sh.n_time != h->n_time) return XCORR_EINVAL;
+    for (int k = 0; k < s->depth; ++k) {
+        if (cudaMalloc(&s->pkt_buf[k], max_packets * (size_t)a->sh.packet_bytes) != cudaSuccess ||
+            cudaMalloc(&s->flags_buf[k], h->frame_bytes / 8) != cudaSuccess ||
+            cudaMalloc(&s->lost_buf[k], sizeof(int32_t) * h->n_freq) != cudaSuccess) {
+            h->last_cuda_error = (int)cudaGetLastError();
+            return XCORR_ENOMEM;
+        }
+    }
+    s->assembler = a;
+    s->max_packets = max_packets;
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_stream_submit_packets(xcorr_stream *s, const void *packets_host, size_t n_packets, uint64_t seq0)
+{
+    if (!s || !s->assembler || (!packets_host && n_packets) || n_packets > s->max_packets) return XCORR_EINVAL;
+    xcorr_handle *h = s->h;
+    xcorr_assembler *a = s->assembler;
+    if (h->samples_since_read + (long long)h->n_time > 16777215ll) return XCORR_EOVERFLOW;
+    const int k = (int)(s->submitted % (unsigned long long)s->depth);
+    if (s->submitted >= (unsigned long long)s->depth) XC_CUDA(h, cudaEventSynchronize(s->consumed[k]));   // ring back-pressure
+    if (n_packets)
+        XC_CUDA(h, cudaMemcpyAsync(s->pkt_buf[k], packets_host, n_packets * (size_t)a->sh.packet_bytes, cudaMemcpyHostToDevice,
+                                   s->copy_stream));
+    XC_CUDA(h, cudaEventRecord(s->copied[k], s->copy_stream));
+    XC_CUDA(h, cudaStreamWaitEvent(s->compute_stream, s->copied[k], 0));
+    int rc = xcorr_assemble(a, s->pkt_buf[k], n_packets, seq0, s->buf[k], s->flags_buf[k], s->lost_buf[k], nullptr, (void *)s->compute_stream);
+    if (rc != XCORR_OK) return rc;
+    rc = xcorr_process(h, s->buf[k], (void *)s->compute_stream);
+    if (rc != XCORR_OK) return rc;
+    if (h->norm) {
+        rc = xcorr_norm_process_dev(h, s->flags_buf[k], s->lost_buf[k], (void *)s->compute_stream);
+        if (rc != XCORR_OK) return rc;
+    }
+    XC_CUDA(h, cudaEventRecord(s->consumed[k], s->compute_stream));
+    s->submitted += 1;
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_stream_read_normalized(xcorr_stream *s, float *vis_out, int32_t *lost_matrix_out)
+{
+    if (!s || !vis_out) return XCORR_EINVAL;
+    const int rc = xcorr_read_normalized(s->h, vis_out, lost_matrix_out, (void *)s->compute_stream);
+    if (rc != XCORR_OK) return rc;
+    XC_CUDA(s->h, cudaStreamSynchronize(s->compute_stream));
     return XCORR_OK;
 }

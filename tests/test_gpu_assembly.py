@@ -129,6 +129,42 @@ def test_packets_to_normalised_visibilities_end_to_end(xb):
     a.close(); x.close()
 
 
+def test_streamed_packet_path(xb):
+    """Pinned packet rings -> xcorr_stream_submit_packets (H2D, assemble, correlate, flag / loss accounting) x 5 frames over a
+    depth-2 ring -> one normalised read; and the same stream without normalisation -> exact int32 visibilities."""
+    n, f, t = 32, 16, 128
+    cases = [make_case(n, f, t, 300 + 7 * k, kind="gaussian", seq0=50_000 + k * t) for k in range(5)]
+    wants = [oa.assemble(arr, n, f, t, seq0) for arr, seq0 in cases]
+    max_pk = max(arr.shape[0] for arr, _ in cases)
+    pinned = [torch.from_numpy(arr.reshape(-1)).pin_memory() for arr, _ in cases]
+    vis_sum = sum(oracle.planar(w["frame"]).astype(np.int64) for w in wants)
+    for norm in (False, True):
+        x = xb.XCorr(n, f, t)
+        if norm:
+            x.norm_enable()
+        a = xb.Assembler(n, f, t)
+        s = xb.XCorrStream(x, depth=2)
+        s.attach_assembler(a, max_pk)
+        for (arr, seq0), p in zip(cases, pinned):
+            s.submit_packets(p, arr.shape[0], seq0)
+        if not norm:
+            out = torch.empty((f, x.n_pairs, 2), dtype=torch.int32).pin_memory()
+            s.read(out)
+            assert np.array_equal(out.numpy(), vis_sum)
+        else:
+            out = torch.empty((f, x.n_pairs, 2), dtype=torch.float32).pin_memory()
+            L = torch.empty((f, x.n_pairs), dtype=torch.int32).pin_memory()
+            s.read_normalized(out, L)
+            flags_all = np.concatenate([np.unpackbits(w["flags"], axis=-1, bitorder="little").astype(bool) for w in wants], axis=0)
+            want_L = on.lost_matrix(flags_all, sum(w["lost"] for w in wants))
+            assert np.array_equal(L.numpy().astype(np.int64), want_L)
+            want_v = on.normalise(vis_sum, 5 * t, want_L)
+            assert np.all(np.abs(out.numpy() - want_v) <= 2.0 ** -22 * np.abs(want_v))
+        # more packets than the ring slots hold
+        assert xb.xcorr_stream_submit_packets(s.stream, pinned[0].data_ptr(), max_pk + 1, 0) == xb.XCORR_EINVAL
+        s.close(); a.close(); x.close()
+
+
 def test_c2_full_size_assembly(xb):
     """BASELINE C2 shape (N=256, F=64, T=16384: 32768 packets of 9248 bytes), the launch configuration bench.py times:
     the whole frame, flag field and counters against what the generator dropped (properties that hold at any size), and
