@@ -1,7 +1,7 @@
 // finalize_kernel.cuh -- xcorr_read's kernel: accumulator slots (layout.hpp) -> packed upper triangle
 // int32[F][P][2] (R4), and the SIMT cross-check kernel used only by the tests.
 //
-// A slot is [r][col/4][row][4] (row = TMEM lane fast), the output is row-major in (i, j).  Each block turns one
+// A slot is [r][row/32][col/4][row%32][4] (layout.hpp), the output is row-major in (i, j).  Each block turns one
 // 32 x 32 patch around through shared memory so that both sides are coalesced: 16-byte vector reads along the row
 // index, 8-byte (re, im) writes along j.  The slots of a super-tile (one per work segment that summed part of
 // its time range) are added here, and the operand offsets are removed (layout.hpp "OFFSET OPERANDS"): with
@@ -29,7 +29,7 @@ __device__ __forceinline__ uint4 slot_sum_v4(const int32_t *__restrict__ acc, in
     for (int sl = slot_begin; sl < slot_end; ++sl) {
         // streaming (evict-first) load: a slot is dead once it has been read here
         const uint4 v = __ldcs(reinterpret_cast<const uint4 *>(acc + (size_t)sl * kAccElemsPerSlot + (size_t)r * kAccElemsPerCta +
-                                                               ((size_t)col4 * kBlock + row) * 4));
+                                                               (size_t)(row >> 5) * kAccElemsPerQuarter + ((size_t)col4 * 32 + (row & 31)) * 4));
         s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
     }
     return s;

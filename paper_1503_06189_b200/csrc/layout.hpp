@@ -6,11 +6,13 @@
 //
 // Device accumulator ("kernels add to the output of the last run").  A super-tile may be summed
 // over time by several work segments (schedule.hpp); every segment owns one SLOT, so the epilogue needs no
-// atomics: it stores (first frame of an integration) or load-add-stores (later frames) its own slot, and
-// xcorr_read adds the slots of a tile together.  Slot layout -- TMEM-native, so that one warp's 16-byte
-// vector accesses are 512-byte contiguous:
+// atomics between segments: it stores (first frame of an integration) or reduce-adds (later frames) into its own slot,
+// and xcorr_read adds the slots of a tile together.  Slot layout -- TMEM-native:
 //
-//   acc[slot][r][col / 4][row][col % 4]   int32,   r in {0,1}, col in [0,512), row in [0,128)
+//   acc[slot][r][row / 32][col / 4][row % 32][col % 4]   int32,   r in {0,1}, col in [0,512), row in [0,128)
+//
+// i.e. per epilogue warp (32 TMEM lanes) the columns run contiguously: a chunk of 32 columns is one 4 KiB piece, which
+// the epilogue stages in shared memory and hands to ONE bulk copy (first frame) or bulk int32 reduce-add (later frames).
 //
 //     row          = TMEM lane       : input  i = 256*I + 128*r + row
 //     col in [0,256)  "R" columns    : input  j = 256*J + col          value  Re V[i,j] = sum h_i h_j + l_i l_j
@@ -42,6 +44,7 @@ constexpr int kBlock = 128;        // inputs per CTA row block (TMEM lanes)
 constexpr int kSuper = 256;        // inputs per super-block (CTA pair)
 constexpr int kAccCols = 512;      // TMEM columns per CTA: 256 R + 256 Q
 constexpr int kAccElemsPerCta = kAccCols * kBlock;          // 65536 int32
+constexpr int kAccElemsPerQuarter = kAccCols * 32;          // 16384 int32: the 32 TMEM lanes one epilogue warp owns
 constexpr int kAccElemsPerSlot = 2 * kAccElemsPerCta;        // 131072 int32 = 512 KiB
 constexpr int kSumPlanes = 4;                                // h'_A, l'_A, h'_B, l'_B
 constexpr int kSumElemsPerCta = kSumPlanes * kBlock;          // 512 int32
@@ -56,7 +59,7 @@ __host__ __device__ inline long long pair_index(long long n, long long i, long l
 // int32 offset of (r, col, row) inside a slot
 __host__ __device__ inline size_t slot_offset(int r, int col, int row)
 {
-    return (size_t)r * kAccElemsPerCta + ((size_t)(col >> 2) * kBlock + row) * 4 + (col & 3);
+    return (size_t)r * kAccElemsPerCta + (size_t)(row >> 5) * kAccElemsPerQuarter + ((size_t)(col >> 2) * 32 + (row & 31)) * 4 + (col & 3);
 }
 
 }  // namespace xc

@@ -207,6 +207,24 @@ __device__ __forceinline__ int4 ld_global_v4(const int32_t *addr)
     return r;
 }
 
+// ---------------------------------------------------------------- bulk (TMA) stores smem -> global, issued by one thread
+__device__ __forceinline__ void bulk_store(void *gdst, uint32_t smem_src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_src), "r"(bytes) : "memory");
+}
+// the same as an int32 add performed at the destination (no load in the SM: the reduction happens in L2)
+__device__ __forceinline__ void bulk_reduce_add_s32(void *gdst, uint32_t smem_src, uint32_t bytes)
+{
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.s32 [%0], [%1], %2;" ::"l"(gdst), "r"(smem_src), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// all but the newest kPending groups of this thread have finished READING their shared-memory source
+template <int kPending>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(kPending) : "memory"); }
+// all groups of this thread have completed (their global writes are done)
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
 // ---------------------------------------------------------------- descriptors
 // Shared-memory matrix descriptor, MN-major, SWIZZLE_128B, int8: the operand tile is rows of 128 bytes
 // (128 MN elements, contiguous), row k at +128*k bytes, 16-byte chunks XOR-swizzled by (k & 7) -- exactly what

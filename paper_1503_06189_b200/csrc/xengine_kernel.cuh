@@ -9,7 +9,8 @@
 //   a3  one thread issues 2-CTA tcgen05.mma kind::i8 (M = 256 over the CTA pair, N = 256, K = 32) with
 //       both operands MN-major straight from those planes; int32 accumulators stay in TMEM (512 columns)
 //       for the whole time range of the work segment
-//   a4  epilogue warps tcgen05.ld the accumulators and add them into this segment's accumulator slot (no atomics)
+//   a4  epilogue warps tcgen05.ld the accumulators, stage them in shared memory and bulk-copy (first frame) or bulk
+//       reduce-add (later frames) them into this segment's accumulator slot
 //
 // Complex product from stacked real GEMMs (BASELINE.json:north_star (b)); h = Re plane, l = Im plane (offset values):
 //   diagonal super-tile (I == J):   R += h h^T ; R += l l^T ; Q += l h^T      (Im V = Q - Q^T, formed at read)
@@ -75,7 +76,9 @@ struct KernelCfg {
     static constexpr int kThreads = (4 + kUnpackWarps + 4) * 32;
     static constexpr int kSumPlanes = 2 * kPackedBlocks;           // column sums kept by the unpack warps: h'_a l'_a [h'_b l'_b]
     static constexpr int kSumScratch = kUnpackThreads * 32;        // cross-thread reduction of the column sums (8 KiB)
-    static constexpr int kSmemData = kPackedStages * kPackedStageBytes + kPlaneStages * kPlaneStageBytes + kSumScratch;
+    static constexpr int kEpiStageBytes = 32 * 32 * 4;             // one chunk of a warp: 32 rows x 32 columns int32 = 4 KiB
+    static constexpr int kEpiStaging = 4 * 2 * kEpiStageBytes;     // 4 epilogue warps x 2 buffers (32 KiB)
+    static constexpr int kSmemData = kPackedStages * kPackedStageBytes + kPlaneStages * kPlaneStageBytes + kSumScratch + kEpiStaging;
     static constexpr int kSmemBytes = kSmemData + 1024 /*align slack*/ + 1024 /*barriers*/;
     // column sums: a thread sees kRowsPerStage rows of its 16 inputs per stage; byte lanes hold 17 rows of values <= 15,
     // 16-bit lanes 4369 rows
@@ -135,7 +138,8 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     const uint32_t smem_packed = smem_base;
     const uint32_t smem_planes = smem_packed + Cfg::kPackedStages * Cfg::kPackedStageBytes;
     const uint32_t smem_sumscratch = smem_planes + Cfg::kPlaneStages * Cfg::kPlaneStageBytes;
-    const uint32_t bar_base = smem_sumscratch + Cfg::kSumScratch;
+    const uint32_t smem_epistage = smem_sumscratch + Cfg::kSumScratch;
+    const uint32_t bar_base = smem_epistage + Cfg::kEpiStaging;
     // barrier slots (8 bytes each)
     auto bar_pk_full = [&](int s) { return bar_base + 8u * (uint32_t)s; };
     auto bar_pk_empty = [&](int s) { return bar_base + 8u * (uint32_t)(Cfg::kPackedStages + s); };
@@ -485,6 +489,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         const uint32_t quarter = warp & 3u;                      // TMEM lanes [32*quarter, 32*quarter+32)
         const uint32_t acc_empty_leader = ptx::mapa(bar_acc_empty, 0);
         uint32_t unit = 0;
+        uint32_t epi_chunks = 0;                                 // chunks this warp has handed to the bulk engine so far
         XC_PROF_DECL(t_epi);
         for (int sg = seg_begin; sg < seg_end; ++sg, ++unit) {
             const Segment seg = p.segments[sg];
@@ -495,7 +500,8 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             const int rows_valid = p.n_inputs - seg.I * kSuper - row0;         // rows of this warp that are real inputs
             const int cols_valid = min(kSuper, p.n_inputs - seg.J * kSuper);   // columns that are real inputs
             // this segment's own slot: [r][col/4][row][4] int32 -> one warp's 16-byte accesses are 512 B contiguous
-            int32_t *slot_cta = p.acc + ((size_t)seg.slot * 2 + rank) * (size_t)kAccElemsPerCta + (size_t)(quarter * 32 + lane) * 4;
+            // this warp's 64 KiB of the segment's own slot: [col / 4][row % 32][4] int32, columns contiguous
+            int32_t *slot_warp = p.acc + ((size_t)seg.slot * 2 + rank) * (size_t)kAccElemsPerCta + (size_t)quarter * kAccElemsPerQuarter;
             // this warp's last TMEM load has landed: the next unit's MMAs may overwrite the accumulators
             bool released = false;
             auto release_tmem = [&]() {
@@ -517,22 +523,28 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 auto chunk_load = [&](int ch, uint32_t (&v)[32]) {
                     ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + (uint32_t)chunk_col(ch), v);
                 };
+                // a chunk leaves through shared memory: 32 lanes x 8 x 16 bytes = the 4 KiB piece of the slot in its final order,
+                // handed to ONE bulk copy (first frame of an integration) or bulk int32 reduce-add (later frames: the addition
+                // happens at the destination, nothing is loaded into the SM).  Two staging buffers per warp; lane 0 owns the
+                // bulk groups.
                 auto chunk_store = [&](int ch, const uint32_t (&v)[32]) {
-                    int32_t *dst = slot_cta + (size_t)(chunk_col(ch) >> 2) * (kBlock * 4);
-                    if (p.first_frame) {
+                    const uint32_t stage = smem_epistage + (quarter * 2u + (uint32_t)(epi_chunks & 1u)) * Cfg::kEpiStageBytes;
+                    if (lane == 0) ptx::bulk_wait_read<1>();       // the copy that last read this buffer (two chunks ago) is done with it
+                    __syncwarp();
 #pragma unroll
-                        for (int g = 0; g < 8; ++g)
-                            ptx::st_global_v4(dst + g * (kBlock * 4), (int32_t)v[4 * g], (int32_t)v[4 * g + 1], (int32_t)v[4 * g + 2],
-                                              (int32_t)v[4 * g + 3]);
-                    } else {
-                        int4 old[8];
-#pragma unroll
-                        for (int g = 0; g < 8; ++g) old[g] = ptx::ld_global_v4(dst + g * (kBlock * 4));
-#pragma unroll
-                        for (int g = 0; g < 8; ++g)
-                            ptx::st_global_v4(dst + g * (kBlock * 4), old[g].x + (int32_t)v[4 * g], old[g].y + (int32_t)v[4 * g + 1],
-                                              old[g].z + (int32_t)v[4 * g + 2], old[g].w + (int32_t)v[4 * g + 3]);
+                    for (int g = 0; g < 8; ++g)
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(stage + (uint32_t)g * 512u + lane * 16u), "r"(v[4 * g]),
+                                     "r"(v[4 * g + 1]), "r"(v[4 * g + 2]), "r"(v[4 * g + 3])
+                                     : "memory");
+                    ptx::fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) {
+                        int32_t *dst = slot_warp + (size_t)(chunk_col(ch) >> 2) * (32 * 4);
+                        if (p.first_frame) ptx::bulk_store(dst, stage, Cfg::kEpiStageBytes);
+                        else ptx::bulk_reduce_add_s32(dst, stage, Cfg::kEpiStageBytes);
+                        ptx::bulk_commit();
                     }
+                    ++epi_chunks;
                 };
                 // two register buffers: the TMEM load of chunk k+1 is in flight while chunk k is written out
                 uint32_t va[32], vb[32];
@@ -551,6 +563,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             if (!released) release_tmem();
             XC_PROF_END(t_epi);
         }
+        if (lane == 0) ptx::bulk_wait_all();                     // the slot is complete in global memory before the grid ends
         if (warp == (uint32_t)Cfg::kWarpEpi0 && lane == 0) XC_PROF_STORE(8, t_epi);
     }
 
