@@ -61,6 +61,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
     __shared__ uint32_t sQ[32][33];   // [col][row]
     __shared__ uint32_t sX[32][33];   // [row j][col i] of the transposed patch (diagonal super-tiles only)
     __shared__ uint32_t sS[4][32];    // column sums: [0] sh_i [1] sl_i (rows of the patch)  [2] sh_j [3] sl_j (columns)
+    __shared__ int32_t sC[2][32];     // kNormalise: flag counters c_f[i] of the patch's rows [0] and columns [1] (the diagonal of X)
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;   // ty in 0..7
     const int nb = n_super(n_inputs), nst = n_supertiles(nb);
     const int i0 = bi * 32, j0 = bj * 32;
@@ -84,6 +85,14 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
             const uint4 vx = slot_sum_v4(acc, sb, se, jl / kBlock, 64 + ((i0 % kSuper) >> 2) + ty, jl % kBlock);
             sX[tx][4 * ty + 0] = vx.x; sX[tx][4 * ty + 1] = vx.y; sX[tx][4 * ty + 2] = vx.z; sX[tx][4 * ty + 3] = vx.w;
         }
+        if constexpr (kNormalise) {
+            // the counters sit on the diagonal of X, one cache line each: fetch them here, beside the slot loads, once per block
+            if (ty >= 4 && ty < 6) {
+                const int nn = ((ty == 4) ? i0 : j0) + tx;
+                const long long PP = (long long)n_inputs * (n_inputs + 1) / 2;
+                sC[ty - 4][tx] = (nn < n_inputs) ? np.x[(long long)f * PP + pair_index(n_inputs, nn, nn)] : 0;
+            }
+        }
         if (ty < 4) {
             // ty 0,1: sh, sl of row input i0 + tx (A block of its CTA half); ty 2,3: of column input j0 + tx
             // (A block again on a diagonal super-tile, the B block for I < J)
@@ -101,7 +110,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
     const uint32_t shj = sS[2][tx], slj = sS[3][tx];
     int32_t x_jj = 0, lost_f = 0;
     if constexpr (kNormalise) {
-        if (j0 + tx < n_inputs) x_jj = np.x[(long long)f * P + pair_index(n_inputs, j0 + tx, j0 + tx)];
+        x_jj = sC[1][tx];
         lost_f = np.lost[f];
     }
     for (int ic = ty; ic < 32; ic += 8) {
@@ -115,7 +124,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
             const long long p = (long long)f * P + pair_index(n_inputs, i, j);
             if constexpr (kNormalise) {
                 // L = lost + c_i + c_j - X_ij (the point (i, i) receives its counter once); V~ = V * T / (T - L)
-                const int32_t x_ii = np.x[(long long)f * P + pair_index(n_inputs, i, i)];
+                const int32_t x_ii = sC[0][ic];
                 int32_t x_ij = 0;
                 if (i != j) {
                     x_ij = np.x[p];
