@@ -229,6 +229,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-next-rows", action="store_true")
+    ap.add_argument("--no-int8-probe", action="store_true")
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
     if args.impl == "reference":
@@ -322,6 +323,31 @@ def main():
         "frac_of_sustained_peak": (achieved / peak_sustained) if peak_sustained else None, "peak_sustained": peak_sustained,
         "hbm_gbs_staging": cfg.frame_bytes / (k_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"],
     }
+
+    # context for the denominator: the library's own int8 GEMM on this box in this run (cuBLAS through torch._int_mm,
+    # 8192^3, best of 10 after 3 warm-ups).  Not used for `frac`; shows where a plain int8 contraction lands on this part.
+    if rank == 0 and not args.no_int8_probe:
+        try:
+            ga = torch.randint(-8, 8, (8192, 8192), dtype=torch.int8, device="cuda")
+            gb = torch.randint(-8, 8, (8192, 8192), dtype=torch.int8, device="cuda")
+            best = None
+            for k in range(13):
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                g0.record()
+                torch._int_mm(ga, gb)
+                g1.record()
+                torch.cuda.synchronize()
+                if k >= 3:
+                    best = g0.elapsed_time(g1) if best is None else min(best, g0.elapsed_time(g1))
+            roofline["cublas_int8_gemm_8192_tops_burst"] = 2.0 * 8192 ** 3 / (best * 1e-3) / 1e12
+            nb = -(-cfg.n_inputs // 256)                       # 256 x 256 super-tiles: 3 MMAs on the diagonal, 4 above it
+            issued_over_useful = (3 * nb + 4 * nb * (nb - 1) // 2) * 65536 / (4.0 * cfg.n_pairs)
+            roofline["issued_over_useful"] = issued_over_useful
+            roofline["issued_int8_tops"] = achieved * issued_over_useful
+            del ga, gb
+        except Exception as e:  # the probe is context only
+            roofline["cublas_int8_gemm_8192_tops_burst"] = None
+            roofline["int8_probe_error"] = str(e)[:120]
 
     # ---- e2e: streamed C-ABI path, HOST frames in, HOST visibilities out, every step
     e2e = None
