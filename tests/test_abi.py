@@ -77,6 +77,10 @@ def test_assembler_null_handles_are_harmless():
     xb.xcorr_assembler_destroy(0)
     assert xb.xcorr_assemble(0, 0, 0, 0, 0) == xb.XCORR_EINVAL
     assert xb.xcorr_norm_process_dev(0, 0, 0, 0) == xb.XCORR_EINVAL
+    assert xb.xcorr_stream_attach_assembler(0, 0, 16) == xb.XCORR_EINVAL
+    assert xb.xcorr_stream_submit_packets(0, 0, 0, 0) == xb.XCORR_EINVAL
+    assert xb.xcorr_stream_read_normalized(0, 0) == xb.XCORR_EINVAL
+    assert xb.xcorr_stream_read_async(0, 0) == xb.XCORR_EINVAL
 
 
 def test_create_fails_loudly_without_a_gpu():
