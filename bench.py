@@ -258,6 +258,7 @@ def main():
     host_frames = [cfg.frame(k) for k in range(n_distinct)]
     dev_frames = [torch.from_numpy(f).cuda() for f in host_frames]
     x = xb.XCorr(cfg.n_inputs, cfg.n_freq, cfg.n_time)
+    x.promise_complete_frames()      # the frames are resident and complete long before any launch (include/xcorr.h)
     out_dev = torch.empty((cfg.n_freq, cfg.n_pairs, 2), dtype=torch.int32, device="cuda")
     st = torch.cuda.Stream()
 
@@ -416,7 +417,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8",
             "data": "synthetic",
             "config": {"workload": cfg.name, "n_inputs": cfg.n_inputs, "n_freq": cfg.n_freq, "t_per_frame": cfg.n_time,
-                       "frame_bytes": cfg.frame_bytes, "step": "xcorr_process + xcorr_read (one integration per frame)",
+                       "frame_bytes": cfg.frame_bytes, "step": "xcorr_process + xcorr_read (one integration per frame)", "options": "xcorr_promise_complete_frames(1)",
                        "l2": f"inputs larger than L2: {n_distinct} distinct {cfg.frame_bytes >> 20} MiB frames alternate",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "note": cfg.note},
             "cmac_per_s": cmac_per_s,

@@ -85,6 +85,21 @@ int xcorr_create(int n_inputs, int n_freq, int t_per_frame, xcorr_handle **out);
 int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void *cuda_stream);
 
 /*
+ * xcorr_promise_complete_frames -- optional promise about the frames handed to xcorr_process() on this handle.
+ *
+ * xengine_kernel is launched with programmatic dependent launch, so it may begin while the previous kernel of the
+ * stream is still finishing.  By default its first frame load therefore waits for that kernel, in case it is the
+ * producer of the frame and signalled launch completion early.  With `enabled` != 0 the caller promises that a frame
+ * is never the output of a kernel that signals programmatic launch completion (cudaTriggerProgrammaticLaunchCompletion /
+ * griddepcontrol.launch_dependents) before it has finished writing it.  Frames that are resident, that arrive by
+ * cudaMemcpy, or that are written by ordinary kernels or by this library's assemble_kernel all qualify.  The frame is then
+ * loaded, unpacked and multiplied while the previous xcorr_read / xcorr_process of the stream drains (C2: about 2 us per
+ * frame); the accumulator is still guarded (the epilogue waits for the previous kernel before it touches a slot).
+ * Errors: EINVAL (NULL handle).
+ */
+int xcorr_promise_complete_frames(xcorr_handle *h, int enabled);
+
+/*
  * xcorr_read -- end the integration: write the visibilities and clear the accumulator (PAPER.md:99:
  * the device-to-host copy happens only at the end of an integration).
  *

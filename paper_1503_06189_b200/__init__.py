@@ -16,7 +16,7 @@ __all__ = [
     "XCORR_OK", "XCORR_EINVAL", "XCORR_EARCH", "XCORR_ENOMEM", "XCORR_ECUDA", "XCORR_EOVERFLOW",
     "XCorrError", "lib", "xcorr_create", "xcorr_process", "xcorr_read", "xcorr_destroy", "xcorr_strerror",
     "xcorr_last_cuda_error", "xcorr_frame_bytes", "xcorr_output_bytes", "xcorr_kernel_launches",
-    "xcorr_norm_enable", "xcorr_norm_process", "xcorr_read_normalized",
+    "xcorr_norm_enable", "xcorr_norm_process", "xcorr_read_normalized", "xcorr_promise_complete_frames",
     "xcorr_stream_create", "xcorr_stream_submit", "xcorr_stream_sync", "xcorr_stream_read", "xcorr_stream_read_async", "xcorr_stream_destroy",
     "xcorr_assembler_create", "xcorr_assembler_packet_bytes", "xcorr_assemble", "xcorr_assembler_kernel_launches",
     "xcorr_assembler_destroy", "xcorr_norm_process_dev", "xcorr_stream_attach_assembler", "xcorr_stream_submit_packets",
@@ -71,6 +71,8 @@ def lib() -> ctypes.CDLL:
     L.xcorr_output_bytes.restype = ctypes.c_size_t
     L.xcorr_kernel_launches.argtypes = [vp]
     L.xcorr_kernel_launches.restype = ctypes.c_uint64
+    L.xcorr_promise_complete_frames.argtypes = [vp, ci]
+    L.xcorr_promise_complete_frames.restype = ci
     L.xcorr_norm_enable.argtypes = [vp]
     L.xcorr_norm_enable.restype = ci
     L.xcorr_norm_process.argtypes = [vp, vp, vp, vp]
@@ -155,6 +157,10 @@ def xcorr_output_bytes(handle: int) -> int:
 
 def xcorr_kernel_launches(handle: int) -> int:
     return lib().xcorr_kernel_launches(handle)
+
+
+def xcorr_promise_complete_frames(handle: int, enabled: int = 1) -> int:
+    return lib().xcorr_promise_complete_frames(handle, int(enabled))
 
 
 def xcorr_norm_enable(handle: int) -> int:
@@ -315,6 +321,10 @@ class XCorr:
             raise ValueError("out must be a contiguous int32 tensor of output_bytes bytes")
         self._check(xcorr_read(self.handle, out.data_ptr(), _stream_handle(stream)), "xcorr_read")
         return out
+
+    def promise_complete_frames(self, enabled: bool = True) -> None:
+        """See xcorr_promise_complete_frames in include/xcorr.h."""
+        self._check(xcorr_promise_complete_frames(self.handle, 1 if enabled else 0), "xcorr_promise_complete_frames")
 
     # ---- lost-sample normalisation (NEXT-1)
     def norm_enable(self) -> None:

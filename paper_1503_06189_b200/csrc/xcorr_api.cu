@@ -41,6 +41,7 @@ struct xcorr_handle {
     int32_t *tile_slot_begin = nullptr;  // device, n_tiles + 1
     int n_slots = 0;
     bool clean = true;               // no frame since create / the last read: the next epilogue stores instead of adding
+    bool frames_complete = false;    // xcorr_promise_complete_frames
     int32_t *staging = nullptr;      // device packed triangle for host reads
     Segment *segments = nullptr;     // device
     int32_t *worker_begin = nullptr; // device
@@ -252,6 +253,7 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
     p.n_inputs = h->n_inputs;
     p.n_freq = h->n_freq;
     p.n_time = h->n_time;
+    p.wait_frame = h->frames_complete ? 0 : 1;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     // programmatic dependent launch: this kernel's prologue (barrier init, TMEM allocation, cluster sync) may overlap the
     // tail of the previous kernel of the stream; the kernel itself waits (griddepcontrol.wait) before touching memory
@@ -366,6 +368,13 @@ static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *
     if (lost_matrix_out && !lost_on_device)
         XC_CUDA(h, cudaMemcpyAsync(lost_matrix_out, h->staging_lost, lost_matrix_bytes, cudaMemcpyDeviceToHost, s));
     if (wait && (!on_device || (lost_matrix_out && !lost_on_device))) XC_CUDA(h, cudaStreamSynchronize(s));
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_promise_complete_frames(xcorr_handle *h, int enabled)
+{
+    if (!h) return XCORR_EINVAL;
+    h->frames_complete = enabled != 0;
     return XCORR_OK;
 }
 

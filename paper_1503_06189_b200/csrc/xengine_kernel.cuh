@@ -104,6 +104,7 @@ struct KernelParams {
     int n_inputs;
     int n_freq;
     int n_time;
+    int wait_frame;                // 1: the TMA lane waits for the previous kernel of the stream before the first frame load
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -194,7 +195,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         ptx::fence_proxy_async_smem();
         // the packed barriers and slots are this CTA's own: start the first loads now, so the frame is already on its
         // way while TMEM is allocated and the cluster synchronises
-        ptx::grid_dependency_wait();                              // the frame may be the previous kernel's output
+        // the frame may be the output of the previous kernel of the stream, which may have let this grid start early:
+        // wait for it, unless the caller has promised complete frames (xcorr_promise_complete_frames)
+        if (p.wait_frame) ptx::grid_dependency_wait();
         for (int sg = seg_begin; sg < seg_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++sg) {
             const Segment seg = p.segments[sg];
             for (int st = seg.stage_begin; st < seg.stage_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++st, ++tma_pre)
@@ -209,7 +212,10 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     __syncthreads();
     ptx::cluster_sync();           // barriers of both CTAs initialised before any remote arrive / multicast commit
     ptx::tc_fence_after_sync();
-    ptx::grid_dependency_wait();   // accumulator / sum slots: the previous kernel of the stream may still read or write them
+    // The accumulator / sum slots may still be read or written by the previous kernel of the stream (xcorr_read's
+    // finalize_kernel, or the previous frame's xengine_kernel): the warps that touch them wait (griddepcontrol.wait) right
+    // before their first access -- the unpack warps before a segment's column sums go out, the epilogue warps before the
+    // first chunk -- so loading, unpacking and multiplying the first segment overlap the previous kernel's tail.
 
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
@@ -462,6 +468,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 if (++since_flush == Cfg::kFlushStages) { flush(off ? 4 : 2); since_flush = 0; since_widen = 0; }
             }
             // segment done: this segment's column sums -> its sum slot (same store / load-add-store rule as the epilogue)
+            ptx::grid_dependency_wait();                           // sum slots: see the note at the prologue
             XC_PROF_BEGIN(t_flush);
             flush(off ? 4 : 2);
             XC_PROF_END(t_flush);
@@ -495,6 +502,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             const Segment seg = p.segments[sg];
             ptx::mbar_wait_cluster(bar_acc_full, unit & 1u);
             ptx::tc_fence_after_sync();
+            ptx::grid_dependency_wait();                           // accumulator slots: see the note at the prologue
             XC_PROF_BEGIN(t_epi);
             const int row0 = (int)(rank * kBlock + quarter * 32);             // first row of this warp inside the super-block
             const int rows_valid = p.n_inputs - seg.I * kSuper - row0;         // rows of this warp that are real inputs

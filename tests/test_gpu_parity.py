@@ -115,6 +115,35 @@ def test_accumulates_across_process_calls_and_read_clears(xb):
     x.close()
 
 
+def test_promise_complete_frames_is_exact(xb):
+    """xcorr_promise_complete_frames: frames are loaded while the previous kernel of the stream drains; same bits.  Covers a
+    read followed at once by the next integration, frames added back to back, and a frame written by torch kernels just before."""
+    n, f, t = 256, 6, 700
+    frames = [wl.uniform_frame(n, f, t, seed=900 + k) for k in range(4)]
+    dev = [torch.from_numpy(fr).cuda() for fr in frames]
+    x = xb.XCorr(n, f, t)
+    x.promise_complete_frames()
+    st = torch.cuda.Stream()
+    outs = [torch.empty((f, x.n_pairs, 2), dtype=torch.int32, device="cuda") for _ in range(3)]
+    with torch.cuda.stream(st):
+        for rep in range(3):                       # process, process, read -- three integrations queued without any host sync
+            x.process(dev[rep], st)
+            x.process(dev[rep + 1], st)
+            x.read(outs[rep], st)
+        # a frame produced on the same stream immediately before xcorr_process (ordinary kernels: qualifies for the promise)
+        made = (dev[0] ^ dev[3]).contiguous()
+        x.process(made, st)
+        last = x.read(None, st)
+    torch.cuda.synchronize()
+    for rep in range(3):
+        want = oracle.planar(frames[rep]).astype(np.int64) + oracle.planar(frames[rep + 1])
+        assert np.array_equal(outs[rep].cpu().numpy(), want)
+    assert np.array_equal(last.cpu().numpy(), oracle.planar(frames[0] ^ frames[3]))
+    x.promise_complete_frames(False)
+    x.process(dev[2]); assert np.array_equal(x.read().cpu().numpy(), oracle.planar(frames[2]))
+    x.close()
+
+
 def test_error_codes_on_device(xb):
     x = xb.XCorr(16, 1, 64)
     buf = torch.zeros(16 * 64 + 16, dtype=torch.uint8, device="cuda")
