@@ -35,7 +35,7 @@ import workloads as wl  # noqa: E402
 NOMINAL_INT8_TOPS = 4500.0  # dense int8, B200 nominal (2x the 2.25 PFLOP/s dense bf16 figure)
 # dram__bytes_read.sum + dram__bytes_write.sum of xengine_kernel<false> for one C2 launch, from the committed
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = {"C2": 277.8e6}   # profiles/r01_ncu_full_bench_c2.md: 268.49 MB read + 9.29 MB written
+NCU_TRAFFIC_BYTES = {"C2": 277.2e6}   # profiles/r01_ncu_full_bench_c2.md: 268.49 MB read + 8.66 MB written
 
 
 def load_peaks():
