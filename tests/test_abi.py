@@ -81,6 +81,7 @@ def test_assembler_null_handles_are_harmless():
     assert xb.xcorr_stream_submit_packets(0, 0, 0, 0) == xb.XCORR_EINVAL
     assert xb.xcorr_stream_read_normalized(0, 0) == xb.XCORR_EINVAL
     assert xb.xcorr_stream_read_async(0, 0) == xb.XCORR_EINVAL
+    assert xb.xcorr_promise_complete_frames(0, 1) == xb.XCORR_EINVAL
 
 
 def test_create_fails_loudly_without_a_gpu():
