@@ -26,7 +26,14 @@
  *   - "dev" pointers are CUDA device pointers on the device that was current at xcorr_create();
  *     "host" pointers are ordinary (preferably page-locked) host pointers.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
- *   - A handle is not thread safe; use it from one host thread at a time.
+ *   - A handle is not thread safe; use it from one host thread at a time, with the device it was created on current
+ *     (a call made while another device is current returns XCORR_EINVAL).
+ *   - Stream order.  The device state of a handle (accumulator, flag / loss accumulators) is ordered by the streams the
+ *     calls are given: calls on the SAME stream run in stream order; a call given ANOTHER stream than the handle's
+ *     previous call first makes that stream wait, on the device (cudaStreamWaitEvent), for everything enqueued so far
+ *     on the previous stream -- so xcorr_process on stream A followed by xcorr_read on stream B is safe and exact.  The
+ *     previous stream must still exist at that point (XCORR_EINVAL if it has been destroyed).  The host-side
+ *     bookkeeping (first frame of an integration, overflow guard, sample count) follows the order of the CALLS.
  *   - Nothing is allocated or freed after xcorr_create()/xcorr_stream_create() return (PAPER.md:49:
  *     "the entire application does not malloc or free any memory outside of startup and shutdown").
  *   - There is no CPU fallback: on a machine without an sm_100 GPU xcorr_create() fails with
@@ -111,7 +118,9 @@ int xcorr_promise_complete_frames(xcorr_handle *h, int enabled);
  *                       xcorr_output_bytes() bytes, 16-byte aligned if on the device.
  *   cuda_stream         stream to order the read on (after the xcorr_process calls it should include).
  *
- * After the read the accumulator is zero and the sample counter used for the overflow guard is reset.
+ * The read ends the integration: the next xcorr_process starts from zero (its epilogue overwrites the accumulator slots
+ * instead of adding to them -- there is no clearing pass), a second xcorr_read without a frame in between returns zeros,
+ * and the sample counter used for the overflow guard is reset.
  * Errors: EINVAL, ECUDA.
  */
 int xcorr_read(xcorr_handle *h, int32_t *upper_triangle_out, void *cuda_stream);
@@ -197,8 +206,9 @@ uint64_t xcorr_kernel_launches(const xcorr_handle *h);
 int xcorr_stream_create(xcorr_handle *h, int depth, xcorr_stream **out);
 
 /*
- * xcorr_stream_submit -- enqueue one host frame: H2D copy into the next device buffer (waiting, on the
- * device, for the correlation that last used that buffer), then xcorr_process on the compute stream.
+ * xcorr_stream_submit -- enqueue one host frame: H2D copy into the next device buffer, then xcorr_process on the
+ * compute stream.  Ring back-pressure: if the correlation that last used that device buffer has not finished, the call
+ * blocks the HOST thread until it has (cudaEventSynchronize).
  * `frame_host` (N*F*T bytes, layout as above) should be page-locked (cudaHostAlloc / cudaHostRegister /
  * torch pin_memory) for the copy to overlap; BORROWED until the matching copy has completed, i.e. until
  * `depth` further submits have returned or xcorr_stream_sync()/xcorr_stream_read() returns.

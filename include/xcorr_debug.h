@@ -1,6 +1,6 @@
 /*
- * xcorr_debug.h -- test-support entry points of libxcorr.so.  NOT part of the product path:
- * xcorr_process()/xcorr_read() never call any of these and nothing dispatches to them.
+ * xcorr_debug.h -- host-logic introspection of libxcorr.so (no GPU needed, no kernels): the work schedule
+ * xcorr_create() builds, for the CPU tests of the decomposition.  xcorr_process()/xcorr_read() never call these.
  */
 #ifndef XCORR_DEBUG_H_
 #define XCORR_DEBUG_H_
@@ -26,13 +26,6 @@ int xcorr_debug_schedule(int n_inputs, int n_freq, int t_per_frame, int n_worker
 
 /* Time samples per pipeline stage. */
 int xcorr_debug_stage_samples(void);
-
-/*
- * Same contract as xcorr_process(), computed by a plain one-thread-per-element SIMT loop (no TMA, no
- * tensor cores).  Used by the GPU tests as an on-device second opinion for whole-matrix comparisons at
- * sizes where the CPU oracle takes minutes; parity itself is always judged against oracle/.
- */
-int xcorr_debug_process_simt(xcorr_handle *h, const void *packed_frame_dev, void *cuda_stream);
 
 #ifdef __cplusplus
 }

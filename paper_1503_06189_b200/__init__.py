@@ -21,7 +21,7 @@ __all__ = [
     "xcorr_assembler_create", "xcorr_assembler_packet_bytes", "xcorr_assemble", "xcorr_assembler_kernel_launches",
     "xcorr_assembler_destroy", "xcorr_norm_process_dev", "xcorr_stream_attach_assembler", "xcorr_stream_submit_packets",
     "xcorr_stream_read_normalized",
-    "xcorr_debug_schedule", "xcorr_debug_stage_samples", "xcorr_debug_process_simt", "XCorr", "XCorrStream", "Assembler",
+    "xcorr_debug_schedule", "xcorr_debug_stage_samples", "XCorr", "XCorrStream", "Assembler",
 ]
 
 XCORR_OK, XCORR_EINVAL, XCORR_EARCH, XCORR_ENOMEM, XCORR_ECUDA, XCORR_EOVERFLOW = 0, -1, -2, -3, -4, -5
@@ -113,8 +113,6 @@ def lib() -> ctypes.CDLL:
     L.xcorr_debug_schedule.restype = ci
     L.xcorr_debug_stage_samples.argtypes = []
     L.xcorr_debug_stage_samples.restype = ci
-    L.xcorr_debug_process_simt.argtypes = [vp, vp, vp]
-    L.xcorr_debug_process_simt.restype = ci
     _lib = L
     return L
 
@@ -262,10 +260,6 @@ def xcorr_debug_schedule(n_inputs: int, n_freq: int, t_per_frame: int, n_workers
     return seg[:n], wb
 
 
-def xcorr_debug_process_simt(handle: int, packed_frame_dev: int, cuda_stream: int = 0) -> int:
-    return lib().xcorr_debug_process_simt(handle, packed_frame_dev, cuda_stream)
-
-
 # ------------------------------------------------------------------------------------------ torch conveniences
 def _stream_handle(stream) -> int:
     if stream is None:
@@ -308,9 +302,6 @@ class XCorr:
         if not frame_dev.is_cuda or not frame_dev.is_contiguous() or frame_dev.numel() * frame_dev.element_size() != self.frame_bytes:
             raise ValueError("frame_dev must be a contiguous CUDA tensor of exactly frame_bytes bytes")
         self._check(xcorr_process(self.handle, frame_dev.data_ptr(), _stream_handle(stream)), "xcorr_process")
-
-    def process_simt_debug(self, frame_dev, stream=None) -> None:
-        self._check(xcorr_debug_process_simt(self.handle, frame_dev.data_ptr(), _stream_handle(stream)), "xcorr_debug_process_simt")
 
     def read(self, out=None, stream=None):
         """Write int32[F][P][2] into ``out`` (CUDA or CPU torch int32 tensor; allocated on the device if None)."""

@@ -1,5 +1,5 @@
 // finalize_kernel.cuh -- xcorr_read's kernel: accumulator slots (layout.hpp) -> packed upper triangle
-// int32[F][P][2] (R4), and the SIMT cross-check kernel used only by the tests.
+// int32[F][P][2] (R4).
 //
 // A slot is [r][row/32][col/4][row%32][4] (layout.hpp), the output is row-major in (i, j).  Each block turns one
 // 32 x 32 patch around through shared memory so that both sides are coalesced: 16-byte vector reads along the row
@@ -150,55 +150,6 @@ __global__ void __launch_bounds__(256) clear_diag_kernel(int32_t *__restrict__ x
     if (k >= (long long)n_inputs * n_freq) return;
     const int f = (int)(k / n_inputs), n = (int)(k % n_inputs);
     x[(long long)f * ((long long)n_inputs * (n_inputs + 1) / 2) + pair_index(n_inputs, n, n)] = 0;
-}
-
-// ------------------------------------------------------------------------------------------------
-// SIMT cross-check ("second opinion" for the GPU tests at sizes where the CPU oracle takes minutes).
-// One thread per accumulator element, plain integer loop over t.  NOT used by xcorr_process.
-// Adds into the FIRST slot of each tile (the caller zeroes all slots at the start of an integration).
-// grid: n_tiles * 2 * (128 / 8) blocks, block 256 threads (thread <-> column), 8 rows per block.
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) simt_reference_kernel(const uint8_t *__restrict__ frame, int32_t *acc,
-                                                             const int32_t *__restrict__ tile_slot_begin, int n_inputs, int n_freq,
-                                                             int n_time)
-{
-    constexpr int kRows = 8;
-    const int nb = n_super(n_inputs), nst = n_supertiles(nb);
-    int b = blockIdx.x;
-    const int rowgrp = b % (kBlock / kRows); b /= (kBlock / kRows);
-    const int r = b % 2; b /= 2;
-    const int tile = b;
-    const int f = tile / nst;
-    int st = tile % nst, I = 0;
-    while (st >= nb - I) { st -= nb - I; ++I; }
-    const int J = I + st;
-    const int col = threadIdx.x;
-    const int j = J * kSuper + col;
-    const bool diag = (I == J);
-    int32_t accR[kRows], accQ[kRows];
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) accR[k] = accQ[k] = 0;
-    const int row_base = rowgrp * kRows;
-    const int i_base = I * kSuper + r * kBlock + row_base;
-    for (int t = 0; t < n_time; ++t) {
-        const uint8_t *line = frame + ((size_t)t * n_freq + f) * n_inputs;
-        const int bjv = (j < n_inputs) ? line[j] : 0;
-        const int hj = (int)(int8_t)(bjv & 0xF0) >> 4, lj = (int)(int8_t)((bjv & 15) << 4) >> 4;
-#pragma unroll
-        for (int k = 0; k < kRows; ++k) {
-            const int i = i_base + k;
-            const int biv = (i < n_inputs) ? line[i] : 0;
-            const int hi = (int)(int8_t)(biv & 0xF0) >> 4, li = (int)(int8_t)((biv & 15) << 4) >> 4;
-            accR[k] += hi * hj + li * lj;
-            accQ[k] += diag ? li * hj : li * hj - hi * lj;
-        }
-    }
-    int32_t *base = acc + (size_t)tile_slot_begin[tile] * kAccElemsPerSlot;
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) {
-        atomicAdd(base + slot_offset(r, col, row_base + k), accR[k]);
-        atomicAdd(base + slot_offset(r, 256 + col, row_base + k), accQ[k]);
-    }
 }
 
 }  // namespace xc

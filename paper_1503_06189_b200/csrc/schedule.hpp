@@ -21,10 +21,7 @@
 
 namespace xc {
 
-#ifndef XC_STAGE_T
-#define XC_STAGE_T 64
-#endif
-constexpr int kStageT = XC_STAGE_T;  // time samples per pipeline stage (MMA K-steps of 32)
+constexpr int kStageT = 64;  // time samples per pipeline stage (MMA K-steps of 32)
 
 struct Segment {          // 32 bytes, read by the kernel
     int32_t f;            // channel

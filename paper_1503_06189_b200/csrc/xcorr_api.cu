@@ -26,6 +26,8 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32
                                     const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+constexpr unsigned long long kMaxTiles = 1ull << 18;
+
 struct xcorr_handle {
     int n_inputs = 0, n_freq = 0, n_time = 0;
     int device = 0;
@@ -62,6 +64,11 @@ struct xcorr_handle {
     int32_t *staging_lost = nullptr; // device int32[F][P] for host reads of the normalisation matrix
     cudaEvent_t lost_used[2] = {nullptr, nullptr};   // recorded after the finalize launch that read the snapshot half
     bool flags_dirty = false;        // flag_x holds counts of the current integration
+    // stream ordering of the handle's device state (accumulator slots, flag / loss accumulators): the stream of the last
+    // call that enqueued work on them; a call on another stream first waits (on the device) for that work
+    cudaStream_t last_stream = nullptr;
+    bool has_last_stream = false;
+    cudaEvent_t order_event = nullptr;
 };
 
 struct xcorr_stream {
@@ -113,6 +120,45 @@ static int validate_shape(int n_inputs, int n_freq, int t_per_frame)
     if (n_inputs > 65536 || n_freq > 65535) return XCORR_EINVAL;
     const unsigned long long bytes = (unsigned long long)n_inputs * (unsigned long long)n_freq * (unsigned long long)t_per_frame;
     if (bytes > (1ull << 40)) return XCORR_EINVAL;
+    // work items (256 x 256 super-tiles): every one owns at least one 512 KiB accumulator slot, and the schedule tables
+    // are built on the host -- refuse shapes whose tables alone would not fit a B200 (kMaxTiles slots = 128 GiB)
+    const unsigned long long nb = ((unsigned long long)n_inputs + kSuper - 1) / kSuper;
+    const unsigned long long tiles = (unsigned long long)n_freq * (nb * (nb + 1) / 2);
+    if (tiles > kMaxTiles) return XCORR_EINVAL;
+    return XCORR_OK;
+}
+
+// make_schedule builds std::vectors: never let an exception cross the C ABI
+static int make_schedule_noexcept(int n_inputs, int n_freq, int t_per_frame, int n_workers, Schedule *out)
+{
+    try {
+        *out = make_schedule(n_inputs, n_freq, t_per_frame, n_workers);
+    } catch (...) {
+        return XCORR_ENOMEM;
+    }
+    return XCORR_OK;
+}
+
+// The handle's device pointers belong to the device that was current at xcorr_create()
+static int check_device(int device)
+{
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess) return XCORR_ECUDA;
+    return cur == device ? XCORR_OK : XCORR_EINVAL;
+}
+
+// Order this call's work after the handle's previous work.  Same stream as last time: stream order does it (and nothing
+// is put between two kernels, so programmatic dependent launch keeps working).  Another stream: record an event behind
+// everything enqueued so far on the previous stream and make the new stream wait for it on the device.
+static int order_after_previous(xcorr_handle *h, cudaStream_t s)
+{
+    if (h->has_last_stream && h->last_stream != s) {
+        cudaError_t e = cudaEventRecord(h->order_event, h->last_stream);
+        if (e != cudaSuccess) { cudaGetLastError(); h->last_cuda_error = (int)e; return XCORR_EINVAL; }   // e.g. that stream was destroyed
+        XC_CUDA(h, cudaStreamWaitEvent(s, h->order_event, 0));
+    }
+    h->last_stream = s;
+    h->has_last_stream = true;
     return XCORR_OK;
 }
 
@@ -132,6 +178,7 @@ extern "C" void xcorr_destroy(xcorr_handle *h)
     cudaFree(h->lost_dev);
     cudaFree(h->staging_lost);
     if (h->lost_pinned) cudaFreeHost(h->lost_pinned);
+    if (h->order_event) cudaEventDestroy(h->order_event);
     for (int k = 0; k < 2; ++k)
         if (h->lost_used[k]) cudaEventDestroy(h->lost_used[k]);
     delete[] h->lost_acc;
@@ -173,7 +220,9 @@ extern "C" int xcorr_create(int n_inputs, int n_freq, int t_per_frame, xcorr_han
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return fail(XCORR_ECUDA);
     h->encode = (PFN_encodeTiled)fn;
 
-    const Schedule sched = make_schedule(n_inputs, n_freq, t_per_frame, h->n_workers);
+    Schedule sched;
+    if ((rc = make_schedule_noexcept(n_inputs, n_freq, t_per_frame, h->n_workers, &sched)) != XCORR_OK) return fail(rc);
+    if (cudaEventCreateWithFlags(&h->order_event, cudaEventDisableTiming) != cudaSuccess) return fail(XCORR_ECUDA);
     h->n_slots = (int)sched.segments.size();
     h->acc_bytes = (size_t)h->n_slots * kAccElemsPerSlot * sizeof(int32_t);
     cudaError_t e;
@@ -211,11 +260,7 @@ static int encode_frame_map(xcorr_handle *h, const void *frame_dev, CUtensorMap 
     // a1: global uint8[T][F][N] seen as a 3-D tensor (n, f, t); one box = 128 inputs x 1 channel x kStageT samples,
     // written to smem as kStageT rows of 128 bytes with the 128-byte swizzle the MMA descriptors expect.
     const cuuint64_t dims[3] = {(cuuint64_t)h->n_inputs, (cuuint64_t)h->n_freq, (cuuint64_t)h->n_time};
-#ifdef XC_EXP_FMAJOR   // timing experiment only (wrong results): frame read as [f][t][n], i.e. contiguous boxes
-    const cuuint64_t strides[2] = {(cuuint64_t)h->n_inputs * (cuuint64_t)h->n_time, (cuuint64_t)h->n_inputs};
-#else
     const cuuint64_t strides[2] = {(cuuint64_t)h->n_inputs, (cuuint64_t)h->n_inputs * (cuuint64_t)h->n_freq};
-#endif
     const cuuint32_t box[3] = {(cuuint32_t)kBlock, 1u, (cuuint32_t)kStageT};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void *>(frame_dev), dims, strides, box, estr,
@@ -241,9 +286,11 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
 {
     int rc = check_process_args(h, packed_frame_dev);
     if (rc != XCORR_OK) return rc;
+    if ((rc = check_device(h->device)) != XCORR_OK) return rc;
     alignas(64) CUtensorMap map;
     rc = encode_frame_map(h, packed_frame_dev, &map);
     if (rc != XCORR_OK) return rc;
+    if ((rc = order_after_previous(h, (cudaStream_t)cuda_stream)) != XCORR_OK) return rc;
     KernelParams p;
     p.segments = h->segments;
     p.worker_begin = h->worker_begin;
@@ -294,8 +341,11 @@ static bool is_device_pointer(const void *ptr)
 static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *lost_matrix_out, void *cuda_stream, bool wait = true)
 {
     cudaStream_t s = (cudaStream_t)cuda_stream;
+    int rc0 = check_device(h->device);
+    if (rc0 != XCORR_OK) return rc0;
     const bool on_device = is_device_pointer(vis_out);
     if (on_device && ((uintptr_t)vis_out & 15u) != 0) return XCORR_EINVAL;
+    if ((rc0 = order_after_previous(h, s)) != XCORR_OK) return rc0;
     void *dst = on_device ? vis_out : (void *)h->staging;
     const bool lost_on_device = lost_matrix_out && is_device_pointer(lost_matrix_out);
     int32_t *lost_dst = !lost_matrix_out ? nullptr : (lost_on_device ? lost_matrix_out : h->staging_lost);
@@ -392,18 +442,37 @@ extern "C" int xcorr_norm_enable(xcorr_handle *h)
     if (!h) return XCORR_EINVAL;
     if (h->norm) return XCORR_OK;
     if (!h->clean) return XCORR_EINVAL;   // startup-time call: not in the middle of an integration
+    int rc = check_device(h->device);
+    if (rc != XCORR_OK) return rc;
     const size_t lost_matrix_bytes = h->output_bytes / 2;
+    // everything or nothing: a failure frees what this call allocated, so a retry starts from scratch
+    auto undo = [&](int code, cudaError_t e) {
+        if (e != cudaSuccess) { h->last_cuda_error = (int)e; cudaGetLastError(); }
+        cudaFree(h->flag_x); h->flag_x = nullptr;
+        cudaFree(h->staging_lost); h->staging_lost = nullptr;
+        cudaFree(h->lost_dev); h->lost_dev = nullptr;
+        cudaFree(h->lost_dev_acc); h->lost_dev_acc = nullptr;
+        if (h->lost_pinned) cudaFreeHost(h->lost_pinned);
+        h->lost_pinned = nullptr;
+        delete[] h->lost_acc; h->lost_acc = nullptr;
+        for (int k = 0; k < 2; ++k) {
+            if (h->lost_used[k]) cudaEventDestroy(h->lost_used[k]);
+            h->lost_used[k] = nullptr;
+        }
+        return code;
+    };
     cudaError_t e;
-    if ((e = cudaMalloc(&h->flag_x, lost_matrix_bytes)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
-    if ((e = cudaMalloc(&h->staging_lost, lost_matrix_bytes)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
-    if ((e = cudaMalloc(&h->lost_dev, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
-    if ((e = cudaMalloc(&h->lost_dev_acc, sizeof(int32_t) * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
-    if ((e = cudaMallocHost(&h->lost_pinned, sizeof(int32_t) * 2 * h->n_freq)) != cudaSuccess) { h->last_cuda_error = e; return XCORR_ENOMEM; }
+    if ((e = cudaMalloc(&h->flag_x, lost_matrix_bytes)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
+    if ((e = cudaMalloc(&h->staging_lost, lost_matrix_bytes)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
+    if ((e = cudaMalloc(&h->lost_dev, sizeof(int32_t) * h->n_freq)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
+    if ((e = cudaMalloc(&h->lost_dev_acc, sizeof(int32_t) * h->n_freq)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
+    if ((e = cudaMallocHost(&h->lost_pinned, sizeof(int32_t) * 2 * h->n_freq)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
     h->lost_acc = new (std::nothrow) long long[h->n_freq]();
-    if (!h->lost_acc) return XCORR_ENOMEM;
-    for (int k = 0; k < 2; ++k) XC_CUDA(h, cudaEventCreateWithFlags(&h->lost_used[k], cudaEventDisableTiming));
-    XC_CUDA(h, cudaMemset(h->flag_x, 0, lost_matrix_bytes));
-    XC_CUDA(h, cudaMemset(h->lost_dev_acc, 0, sizeof(int32_t) * h->n_freq));
+    if (!h->lost_acc) return undo(XCORR_ENOMEM, cudaSuccess);
+    for (int k = 0; k < 2; ++k)
+        if ((e = cudaEventCreateWithFlags(&h->lost_used[k], cudaEventDisableTiming)) != cudaSuccess) return undo(XCORR_ECUDA, e);
+    if ((e = cudaMemset(h->flag_x, 0, lost_matrix_bytes)) != cudaSuccess) return undo(XCORR_ECUDA, e);
+    if ((e = cudaMemset(h->lost_dev_acc, 0, sizeof(int32_t) * h->n_freq)) != cudaSuccess) return undo(XCORR_ECUDA, e);
     h->norm = true;
     return XCORR_OK;
 }
@@ -414,6 +483,9 @@ extern "C" int xcorr_norm_process_dev(xcorr_handle *h, const uint8_t *flags_dev,
 {
     if (!h || !h->norm) return XCORR_EINVAL;
     if (flags_dev && ((uintptr_t)flags_dev & 15u) != 0) return XCORR_EINVAL;
+    int rc = check_device(h->device);
+    if (rc != XCORR_OK) return rc;
+    if ((flags_dev || lost_samples_dev) && (rc = order_after_previous(h, (cudaStream_t)cuda_stream)) != XCORR_OK) return rc;
     if (lost_samples_dev) {
         lost_add_kernel<<<(h->n_freq + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(lost_samples_dev, h->lost_dev_acc, h->n_freq);
         XC_CUDA(h, cudaGetLastError());
@@ -431,6 +503,11 @@ extern "C" int xcorr_norm_process(xcorr_handle *h, const uint8_t *flags_dev, con
         for (int f = 0; f < h->n_freq; ++f)
             if (lost_samples_host[f] < 0 || lost_samples_host[f] > h->n_time) return XCORR_EINVAL;
         for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] += lost_samples_host[f];
+    }
+    if (flags_dev) {
+        int rc = check_device(h->device);
+        if (rc != XCORR_OK) return rc;
+        if ((rc = order_after_previous(h, (cudaStream_t)cuda_stream)) != XCORR_OK) return rc;
     }
     return launch_flag_count(h, flags_dev, cuda_stream);
 }
@@ -548,7 +625,8 @@ extern "C" int xcorr_debug_schedule(int n_inputs, int n_freq, int t_per_frame, i
                                     int32_t *worker_begin_out)
 {
     if (validate_shape(n_inputs, n_freq, t_per_frame) != XCORR_OK || n_workers <= 0) return XCORR_EINVAL;
-    const Schedule sched = make_schedule(n_inputs, n_freq, t_per_frame, n_workers);
+    Schedule sched;
+    if (make_schedule_noexcept(n_inputs, n_freq, t_per_frame, n_workers, &sched) != XCORR_OK) return XCORR_ENOMEM;
     const int n = (int)sched.segments.size();
     if (segments_out && worker_begin_out) {
         if (n > max_segments) return XCORR_EINVAL;
@@ -563,32 +641,6 @@ extern "C" int xcorr_debug_schedule(int n_inputs, int n_freq, int t_per_frame, i
 }
 
 extern "C" int xcorr_debug_stage_samples(void) { return kStageT; }
-
-extern "C" int xcorr_debug_process_simt(xcorr_handle *h, const void *packed_frame_dev, void *cuda_stream)
-{
-    int rc = check_process_args(h, packed_frame_dev);
-    if (rc != XCORR_OK) return rc;
-    const int blocks = h->n_tiles * 2 * (kBlock / 8);
-    if (h->clean) {
-        XC_CUDA(h, cudaMemsetAsync(h->acc, 0, h->acc_bytes, (cudaStream_t)cuda_stream));
-        XC_CUDA(h, cudaMemsetAsync(h->sums, 0, h->sums_bytes, (cudaStream_t)cuda_stream));
-    }
-    simt_reference_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const uint8_t *)packed_frame_dev, h->acc, h->tile_slot_begin,
-                                                                            h->n_inputs, h->n_freq, h->n_time);
-    XC_CUDA(h, cudaGetLastError());
-    h->launches += 1;
-    h->samples_since_read += h->n_time;
-    h->clean = false;
-    return XCORR_OK;
-}
-
-#ifdef XC_PROFILE
-// development builds only (-DXC_PROFILE): per-CTA stall counters of the last xengine_kernel launch, [1024][16] uint64
-extern "C" int xcorr_debug_read_profile(unsigned long long *out)
-{
-    return cudaMemcpyFromSymbol(out, g_prof, sizeof(unsigned long long) * 1024 * 16) == cudaSuccess ? XCORR_OK : XCORR_ECUDA;
-}
-#endif
 
 // ---------------------------------------------------------------------------------------------------
 // packet -> frame assembly (NEXT-2; include/xcorr_assemble.h)
@@ -642,7 +694,9 @@ extern "C" int xcorr_assembler_create(int n_inputs, int n_freq, int t_per_frame,
     a->sh.n_streams = n_freq / C; a->sh.n_blocks = t_per_frame / S;
     const unsigned long long pay = (unsigned long long)S * C * n_inputs;
     a->sh.packet_bytes = kPacketHeaderBytes + pay + pay / 8;
-    a->n_positions = (unsigned)a->sh.n_streams * (unsigned)a->sh.n_blocks;
+    const unsigned long long n_pos = (unsigned long long)a->sh.n_streams * (unsigned long long)a->sh.n_blocks;
+    if (n_pos == 0 || n_pos > 0x7FFFFFFFull) { delete a; return XCORR_EINVAL; }
+    a->n_positions = (unsigned)n_pos;
     cudaError_t e;
     if ((e = cudaMalloc(&a->owner, sizeof(uint32_t) * 2 * (size_t)a->n_positions)) != cudaSuccess ||
         (e = cudaMalloc(&a->counts, sizeof(uint32_t) * 8)) != cudaSuccess) {
@@ -667,10 +721,13 @@ extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_
         ((uintptr_t)counts_dev & 3u))
         return XCORR_EINVAL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
+    {
+        const int rc = check_device(a->device);
+        if (rc != XCORR_OK) return rc;
+    }
     // no memsets: the ownership tables and counters are left clean by the previous call's assemble_kernel (see create)
     uint32_t *owner = a->owner + (size_t)(a->calls & 1u) * a->n_positions;
     uint32_t *owner_next = a->owner + (size_t)((a->calls + 1) & 1u) * a->n_positions;
-    a->calls += 1;
     {
         size_t n_threads = n_packets > (size_t)a->sh.n_freq ? n_packets : (size_t)a->sh.n_freq;   // also zeroes lost_dev[F]
         packet_claim_kernel<<<(unsigned)((n_threads + 255) / 256), 256, 0, s>>>((const uint8_t *)packets, (unsigned)n_packets, seq0, a->sh,
@@ -685,6 +742,7 @@ extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_
                                            a->counts, counts_dev);
     XC_CUDA(a, cudaGetLastError());
     a->launches += 1;
+    a->calls += 1;   // the tables swap roles only once both kernels are in the stream
     return XCORR_OK;
 }
 

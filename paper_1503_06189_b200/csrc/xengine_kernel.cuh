@@ -31,20 +31,6 @@
 
 namespace xc {
 
-// Optional stall accounting (development builds only, -DXC_PROFILE): per-CTA cycle counters of where each role waits.
-#ifdef XC_PROFILE
-__device__ unsigned long long g_prof[1024][16];
-#define XC_PROF_DECL(v) long long v = 0
-#define XC_PROF_BEGIN(v) const long long v##_t0 = clock64()
-#define XC_PROF_END(v) v += clock64() - v##_t0
-#define XC_PROF_STORE(idx, v) g_prof[blockIdx.x][idx] = (unsigned long long)(v)
-#else
-#define XC_PROF_DECL(v)
-#define XC_PROF_BEGIN(v)
-#define XC_PROF_END(v)
-#define XC_PROF_STORE(idx, v)
-#endif
-
 // ------------------------------------------------------------------------------------------------
 // compile-time configuration
 // ------------------------------------------------------------------------------------------------
@@ -56,21 +42,9 @@ struct KernelCfg {
     static constexpr int kPlanes = kOffDiag ? 5 : 2;               // h_a l_a [h_b l_b 15-l_b]
     static constexpr int kPackedStageBytes = kPackedBlocks * kPlaneBytes;
     static constexpr int kPlaneStageBytes = kPlanes * kPlaneBytes;
-#ifndef XC_PACKED_STAGES_DIAG
-#define XC_PACKED_STAGES_DIAG 4
-#endif
-#ifndef XC_PLANE_STAGES_DIAG
-#define XC_PLANE_STAGES_DIAG 6
-#endif
-    static constexpr int kPackedStages = kOffDiag ? 3 : XC_PACKED_STAGES_DIAG;
-    static constexpr int kPlaneStages = kOffDiag ? 3 : XC_PLANE_STAGES_DIAG;
-#ifndef XC_UNPACK_WARPS_OFFDIAG
-#define XC_UNPACK_WARPS_OFFDIAG 8
-#endif
-#ifndef XC_UNPACK_WARPS_DIAG
-#define XC_UNPACK_WARPS_DIAG 8
-#endif
-    static constexpr int kUnpackWarps = kOffDiag ? XC_UNPACK_WARPS_OFFDIAG : XC_UNPACK_WARPS_DIAG;   // multiple of 4
+    static constexpr int kPackedStages = kOffDiag ? 3 : 4;
+    static constexpr int kPlaneStages = kOffDiag ? 3 : 6;
+    static constexpr int kUnpackWarps = 8;                         // multiple of 4
     static constexpr int kUnpackThreads = kUnpackWarps * 32;
     static constexpr int kWarpEpi0 = 4 + kUnpackWarps;             // epilogue warps: warp % 4 == TMEM lane quarter
     static constexpr int kThreads = (4 + kUnpackWarps + 4) * 32;
@@ -127,11 +101,6 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     const uint32_t warp = threadIdx.x >> 5;
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t rank = ptx::cluster_ctarank();          // 0 = leader (issues the MMAs)
-#ifdef XC_PROFILE
-    const long long prof_c0 = clock64();
-    unsigned long long prof_g0;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(prof_g0));
-#endif
     const uint32_t worker = blockIdx.x >> 1;
 
     // ---- shared memory carve-up (1024-byte aligned data, then barriers) ----
@@ -224,20 +193,16 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         // ===================================================== a1: TMA producer (one lane)
         if (lane == 0) {
             uint32_t it = 0;
-            XC_PROF_DECL(w_pk_empty);
             for (int sg = seg_begin; sg < seg_end; ++sg) {
                 const Segment seg = p.segments[sg];
                 for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
                     if (it < tma_pre) continue;                    // already in flight (prologue)
                     const uint32_t slot = it % Cfg::kPackedStages;
                     const uint32_t ph = (it / Cfg::kPackedStages) & 1u;
-                    XC_PROF_BEGIN(w_pk_empty);
                     ptx::mbar_wait(bar_pk_empty(slot), ph ^ 1u);
-                    XC_PROF_END(w_pk_empty);
                     tma_issue(seg, st, slot);
                 }
             }
-            XC_PROF_STORE(0, w_pk_empty);
         }
     } else if (warp == kWarpMma) {
         // ===================================================== a3: MMA issuer (leader CTA, one lane)
@@ -246,32 +211,16 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             const uint32_t tmem_R = tmem_base;
             const uint32_t tmem_Q = tmem_base + 256;
             uint32_t it = 0, unit = 0;
-            XC_PROF_DECL(w_acc_empty);
-            XC_PROF_DECL(w_pl_full);
-            XC_PROF_DECL(t_mma);
-            XC_PROF_BEGIN(t_mma);
             for (int sg = seg_begin; sg < seg_end; ++sg, ++unit) {
                 const Segment seg = p.segments[sg];
                 const bool off = kOffDiag && (seg.I != seg.J);
-                XC_PROF_BEGIN(w_acc_empty);
                 ptx::mbar_wait_cluster(bar_acc_empty, (unit & 1u) ^ 1u);     // epilogues of both CTAs drained TMEM
-                XC_PROF_END(w_acc_empty);
                 ptx::tc_fence_after_sync();
                 for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
                     const uint32_t slot = it % Cfg::kPlaneStages;
                     const uint32_t ph = (it / Cfg::kPlaneStages) & 1u;
-                    XC_PROF_BEGIN(w_pl_full);
                     ptx::mbar_wait_cluster(bar_pl_full(slot), ph);
-                    XC_PROF_END(w_pl_full);
                     ptx::tc_fence_after_sync();
-#ifdef XC_PROFILE
-                    if (it == 0) {
-                        unsigned long long g;
-                        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
-                        g_prof[blockIdx.x][13] = (unsigned long long)(clock64() - prof_c0);
-                        g_prof[blockIdx.x][14] = g - prof_g0;
-                    }
-#endif
                     const uint32_t pl = smem_planes + slot * Cfg::kPlaneStageBytes;
 #pragma unroll
                     for (int k = 0; k < kStageT / 32; ++k) {
@@ -280,26 +229,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                         const uint64_t d_la = ptx::make_smem_desc_mn_sw128(pl + 1 * Cfg::kPlaneBytes + koff, 1024, 1024);
                         const uint32_t acc = (st != seg.stage_begin || k != 0) ? 1u : 0u;
                         if (!off) {
-#ifdef XC_EXP_NOMMA   // power experiment only (wrong results): no MMAs issued
-                            (void)acc; (void)d_ha; (void)d_la;
-#elif defined(XC_EXP_N128)   // timing experiment only (wrong results): same tensor work as N = 128 halves, A read twice
-                            constexpr uint32_t idesc_h = ptx::make_idesc_i8_mnmajor(256, 128);
-                            ptx::mma_i8<2>(tmem_R, d_ha, d_ha, idesc_h, acc);
-                            ptx::mma_i8<2>(tmem_R + 128, d_ha, d_ha, idesc_h, acc);
-                            ptx::mma_i8<2>(tmem_R, d_la, d_la, idesc_h, 1u);
-                            ptx::mma_i8<2>(tmem_R + 128, d_la, d_la, idesc_h, 1u);
-                            ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc_h, acc);
-                            ptx::mma_i8<2>(tmem_Q + 128, d_la, d_ha, idesc_h, acc);
-#elif defined(XC_EXP_2P5)   // timing experiment only (wrong results): 2.5 MMAs per K-step
-                            constexpr uint32_t idesc_h = ptx::make_idesc_i8_mnmajor(256, 128);
-                            ptx::mma_i8<2>(tmem_R, d_ha, d_ha, idesc, acc);
-                            ptx::mma_i8<2>(tmem_R, d_la, d_la, idesc_h, 1u);
-                            ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc, acc);
-#else
                             ptx::mma_i8<2>(tmem_R, d_ha, d_ha, idesc, acc);   // R  = h h^T
                             ptx::mma_i8<2>(tmem_R, d_la, d_la, idesc, 1u);    // R += l l^T
                             ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc, acc);   // Q  = l h^T
-#endif
                         } else {
                             const uint64_t d_hb = ptx::make_smem_desc_mn_sw128(pl + 2 * Cfg::kPlaneBytes + koff, 1024, 1024);
                             const uint64_t d_lb = ptx::make_smem_desc_mn_sw128(pl + 3 * Cfg::kPlaneBytes + koff, 1024, 1024);
@@ -314,17 +246,6 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 }
                 ptx::mma_commit<2>(bar_acc_full, 0x3);             // accumulators complete (both CTAs)
             }
-            XC_PROF_END(t_mma);
-#ifdef XC_PROFILE
-            {
-                unsigned long long g;
-                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
-                g_prof[blockIdx.x][15] = g - prof_g0;
-            }
-#endif
-            XC_PROF_STORE(1, w_acc_empty);
-            XC_PROF_STORE(2, w_pl_full);
-            XC_PROF_STORE(3, t_mma);
         }
     } else if (warp >= kWarpUnpack0 && warp < (uint32_t)Cfg::kWarpEpi0) {
         // ===================================================== a2: unpack warps
@@ -390,11 +311,6 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             }
         };
         uint32_t it = 0;
-        XC_PROF_DECL(w_pk_full);
-        XC_PROF_DECL(w_pl_empty);
-        XC_PROF_DECL(t_flush);
-        XC_PROF_DECL(t_unpack);
-        XC_PROF_BEGIN(t_unpack);
         for (int sg = seg_begin; sg < seg_end; ++sg) {
             const Segment seg = p.segments[sg];
             const bool off = kOffDiag && (seg.I != seg.J);
@@ -402,17 +318,10 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
                 const uint32_t pslot = it % Cfg::kPackedStages, pph = (it / Cfg::kPackedStages) & 1u;
                 const uint32_t lslot = it % Cfg::kPlaneStages, lph = (it / Cfg::kPlaneStages) & 1u;
-                XC_PROF_BEGIN(w_pk_full);
                 ptx::mbar_wait(bar_pk_full(pslot), pph);                      // TMA bytes landed
-                XC_PROF_END(w_pk_full);
-                XC_PROF_BEGIN(w_pl_empty);
                 ptx::mbar_wait_cluster(bar_pl_empty(lslot), lph ^ 1u);        // MMAs that read this plane slot retired
-                XC_PROF_END(w_pl_empty);
                 const uint32_t src = smem_packed + pslot * Cfg::kPackedStageBytes;
                 const uint32_t dst = smem_planes + lslot * Cfg::kPlaneStageBytes;
-#ifdef XC_EXP_NOUNPACK   // power experiment only (wrong results): planes are never written
-                if (false)
-#endif
 #pragma unroll
                 for (int q = 0; q < Cfg::kRowsPerStage; ++q) {
                     const uint32_t o = (uint32_t)(q * Cfg::kUnpackThreads + tid) * 16u;
@@ -469,9 +378,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             }
             // segment done: this segment's column sums -> its sum slot (same store / load-add-store rule as the epilogue)
             ptx::grid_dependency_wait();                           // sum slots: see the note at the prologue
-            XC_PROF_BEGIN(t_flush);
             flush(off ? 4 : 2);
-            XC_PROF_END(t_flush);
             if (tid < 128) {
                 int32_t *dst_sum = p.sums + ((size_t)seg.slot * 2 + rank) * (size_t)kSumElemsPerCta + tid;
 #pragma unroll
@@ -484,12 +391,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 }
             }
         }
-        XC_PROF_END(t_unpack);
         if (tid == 0) {
-            XC_PROF_STORE(4, w_pk_full);
-            XC_PROF_STORE(5, w_pl_empty);
-            XC_PROF_STORE(6, t_flush);
-            XC_PROF_STORE(7, t_unpack);
         }
     } else if (warp >= (uint32_t)Cfg::kWarpEpi0) {
         // ===================================================== a4: epilogue warps
@@ -497,13 +399,11 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         const uint32_t acc_empty_leader = ptx::mapa(bar_acc_empty, 0);
         uint32_t unit = 0;
         uint32_t epi_chunks = 0;                                 // chunks this warp has handed to the bulk engine so far
-        XC_PROF_DECL(t_epi);
         for (int sg = seg_begin; sg < seg_end; ++sg, ++unit) {
             const Segment seg = p.segments[sg];
             ptx::mbar_wait_cluster(bar_acc_full, unit & 1u);
             ptx::tc_fence_after_sync();
             ptx::grid_dependency_wait();                           // accumulator slots: see the note at the prologue
-            XC_PROF_BEGIN(t_epi);
             const int row0 = (int)(rank * kBlock + quarter * 32);             // first row of this warp inside the super-block
             const int rows_valid = p.n_inputs - seg.I * kSuper - row0;         // rows of this warp that are real inputs
             const int cols_valid = min(kSuper, p.n_inputs - seg.J * kSuper);   // columns that are real inputs
@@ -518,11 +418,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 if (lane == 0) ptx::mbar_arrive_cluster(acc_empty_leader);
                 released = true;
             };
-#ifdef XC_DEBUG_SKIP_EPI
-            if (false) {
-#else
             if (rows_valid > 0) {
-#endif
                 // R columns: on a diagonal super-tile only j >= i is ever read -> start at this warp's first row
                 const int r_begin = (seg.I == seg.J) ? row0 : 0;
                 const int n_chunks_r = max((cols_valid - r_begin + 31) / 32, 0);
@@ -569,10 +465,8 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 }
             }
             if (!released) release_tmem();
-            XC_PROF_END(t_epi);
         }
         if (lane == 0) ptx::bulk_wait_all();                     // the slot is complete in global memory before the grid ends
-        if (warp == (uint32_t)Cfg::kWarpEpi0 && lane == 0) XC_PROF_STORE(8, t_epi);
     }
 
     // ---- teardown: everyone in both CTAs done with TMEM / peer smem before dealloc and exit ----
@@ -583,16 +477,6 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         ptx::tc_fence_after_sync();
         ptx::tmem_dealloc<2>(tmem_base, kAccCols);
     }
-#ifdef XC_PROFILE
-    if (threadIdx.x == 0) {
-        unsigned long long prof_g1;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(prof_g1));
-        g_prof[blockIdx.x][9] = (unsigned long long)(clock64() - prof_c0);
-        g_prof[blockIdx.x][10] = prof_g1 - prof_g0;
-        g_prof[blockIdx.x][11] = prof_g0;
-        g_prof[blockIdx.x][12] = prof_g1;
-    }
-#endif
 }
 
 }  // namespace xc

@@ -129,7 +129,36 @@ def test_packets_to_normalised_visibilities_end_to_end(xb):
     a.close(); x.close()
 
 
-def test_streamed_packet_path(xb):
+def test_assemble_then_process_with_promise_on_one_stream(xb):
+    """xcorr_promise_complete_frames with the frame written by assemble_kernel immediately before xcorr_process on the same
+    stream (assemble_kernel never signals early launch completion, so it qualifies): several frames back to back into one
+    ring of two frame buffers, every result exact.  Shape with several work segments per worker."""
+    n, f, t = 256, 160, 192
+    cases = [make_case(n, f, t, 700 + 3 * k, kind="gaussian", seq0=90_000 + k * t) for k in range(4)]
+    wants = [oa.assemble(arr, n, f, t, seq0) for arr, seq0 in cases]
+    pk = [torch.from_numpy(arr.reshape(-1)).cuda() for arr, _ in cases]
+    a = xb.Assembler(n, f, t)
+    x = xb.XCorr(n, f, t)
+    x.promise_complete_frames()
+    st = torch.cuda.Stream()
+    bufs = [(torch.empty((t, f, n), dtype=torch.uint8, device="cuda"), torch.empty((t, f, n // 8), dtype=torch.uint8, device="cuda"))
+            for _ in range(2)]
+    outs = []
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        for k, (arr, seq0) in enumerate(cases):
+            frame, flags = bufs[k % 2]
+            a.assemble(pk[k], arr.shape[0], seq0, frame=frame, flags=flags, stream=st)
+            x.process(frame, st)
+            outs.append(x.read(None, st))
+    torch.cuda.synchronize()
+    for w, o in zip(wants, outs):
+        assert np.array_equal(o.cpu().numpy(), oracle.planar(w["frame"]))
+    a.close(); x.close()
+
+
+@pytest.mark.parametrize("promise", [False, True])
+def test_streamed_packet_path(xb, promise):
     """Pinned packet rings -> xcorr_stream_submit_packets (H2D, assemble, correlate, flag / loss accounting) x 5 frames over a
     depth-2 ring -> one normalised read; and the same stream without normalisation -> exact int32 visibilities."""
     n, f, t = 32, 16, 128
@@ -140,6 +169,8 @@ def test_streamed_packet_path(xb):
     vis_sum = sum(oracle.planar(w["frame"]).astype(np.int64) for w in wants)
     for norm in (False, True):
         x = xb.XCorr(n, f, t)
+        if promise:
+            x.promise_complete_frames()
         if norm:
             x.norm_enable()
         a = xb.Assembler(n, f, t)

@@ -47,8 +47,14 @@ def check_vis(got, want):
 
 
 @pytest.mark.parametrize("n,f,t,dense", [(16, 4, 256, True), (48, 3, 100, True), (144, 1, 65, True), (256, 8, 512, False),
-                                         (272, 2, 257, True), (512, 2, 200, False)])
+                                         (272, 2, 257, True), (512, 2, 200, False),
+                                         # several work segments per worker (3 at most, 2 at least on 74 workers): the slots of a
+                                         # tile are summed and normalised in one pass
+                                         (256, 160, 192, False), (512, 60, 192, True)])
 def test_normalisation_matches_oracle(xb, n, f, t, dense):
+    if (n, f, t) in ((256, 160, 192), (512, 60, 192)):
+        _, wb = xb.xcorr_debug_schedule(n, f, t, 74)
+        assert np.diff(wb).max() >= 3
     kw = dict(p_flag=0.03, p_burst=0.05, burst_frac=0.2, p_packet_loss=0.08) if dense else {}
     flags, lost_mask, lost = wl.draw_flags_and_loss(n, f, t, 21, **kw)
     fr = wl.zero_lost_samples(wl.make_frame("gaussian", n, f, t, 22), flags, lost_mask)

@@ -1,10 +1,13 @@
 """GPU parity: the CUDA path (through the C ABI via the thin binding) against the CPU oracle, bit for bit.
 
 Integer work -> the bar is exact equality (np.array_equal), no tolerance.  Small and medium shapes are compared
-element by element against oracle.planar / oracle.naive on the same seeded bytes; BASELINE.json's full-size
-configs are checked (a) on sampled pairs computed one by one by oracle.pairs, (b) by the O(N*T) exact identities
-of oracle/ (total power, Freivalds probes) over every channel, and (c) whole-matrix against the on-device SIMT
-second opinion, which is itself held to (a) and (b).
+element by element against oracle.planar / oracle.naive on the same seeded bytes -- including shapes whose work
+schedule gives every worker several segments (asserted), run as one frame, as three accumulated frames and with
+xcorr_promise_complete_frames.  BASELINE.json's full-size configs are checked (a) element by element against
+oracle.planar on whole channels (all 64 of C2; channels from both the data-parallel and the water-filled part of the
+schedule for C4, C5, C3), (b) on sampled pairs computed one by one by oracle.pairs, (c) by the O(N*T) exact identities
+of oracle/ (total power, Freivalds probes), and, as an extra, (d) whole-matrix against the standalone SIMT second opinion
+of tests/support (which shares no code with libxcorr.so).
 """
 import numpy as np
 import pytest
@@ -24,15 +27,36 @@ def xb():
     return m
 
 
-def run_gpu(xb, frames, simt=False, host_out=False):
+def n_workers():
+    return torch.cuda.get_device_properties(0).multi_processor_count // 2
+
+
+def segments_per_worker(xb, n, f, t):
+    """(max, min) number of work segments any worker gets in the launch configuration of this GPU."""
+    _, wb = xb.xcorr_debug_schedule(n, f, t, n_workers())
+    per = np.diff(wb)
+    return int(per.max()), int(per.min())
+
+
+def run_simt(frame):
+    """The standalone SIMT second opinion (tests/support/simt_xcorr.cu) on one frame -> int32 [F][P][2]."""
+    from tests import support
+    out = support.simt_xcorr(torch.from_numpy(frame).cuda())
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def run_gpu(xb, frames, host_out=False, promise=False):
     """process every frame in `frames` (list of uint8 [T][F][N] numpy arrays), then read."""
     t, f, n = frames[0].shape
     x = xb.XCorr(n, f, t)
+    if promise:
+        x.promise_complete_frames()
     st = torch.cuda.Stream()
     with torch.cuda.stream(st):
         for fr in frames:
             d = torch.from_numpy(fr).cuda()
-            (x.process_simt_debug if simt else x.process)(d, st)
+            x.process(d, st)
         if host_out:
             out = torch.empty((f, x.n_pairs, 2), dtype=torch.int32).pin_memory()
             x.read(out, st)
@@ -69,6 +93,49 @@ EDGE_SHAPES = [
 def test_edge_shapes_exact(xb, n, f, t, kind):
     fr = wl.make_frame(kind, n, f, t, seed=n + 7 * f + t)
     assert np.array_equal(run_gpu(xb, [fr]), oracle.planar(fr))
+
+
+# Shapes whose schedule (xcorr_debug_schedule at this GPU's worker count) gives EVERY worker several segments, so the
+# accumulator hand-off between segments (TMEM full/empty phases), the TMA prologue crossing a segment boundary, the
+# water-filled split of an item along time and, for N > 256, diagonal <-> off-diagonal transitions inside one worker are
+# all exercised -- and compared whole-output, element by element, with the oracle.
+MULTI_SEGMENT_SHAPES = [
+    # (N, F, T, kind, min segments per worker expected on 74 workers)
+    (256, 160, 192, "gaussian", 2), (256, 300, 100, "uniform", 4), (256, 200, 640, "gaussian", 2),
+    (512, 60, 192, "gaussian_sky", 2), (768, 40, 130, "uniform", 3), (1024, 12, 200, "stress", 1),
+]
+
+
+@pytest.mark.parametrize("mode", ["single", "accumulate3", "promise"])
+@pytest.mark.parametrize("n,f,t,kind,min_seg", MULTI_SEGMENT_SHAPES)
+def test_multi_segment_schedules_exact(xb, n, f, t, kind, min_seg, mode):
+    smax, smin = segments_per_worker(xb, n, f, t)
+    if n_workers() == 74:
+        assert smax >= 3 and smin >= min_seg, (smax, smin)
+    if mode == "single":
+        fr = wl.make_frame(kind, n, f, t, seed=11 * n + f + t)
+        assert np.array_equal(run_gpu(xb, [fr]), oracle.planar(fr))
+        return
+    frames = [wl.make_frame(kind, n, f, t, seed=11 * n + f + t + 1000 * (k + 1)) for k in range(3)]
+    want = sum(oracle.planar(fr).astype(np.int64) for fr in frames)
+    if mode == "accumulate3":       # frames 2 and 3 take the cp.reduce.async.bulk path into slots written by frame 1
+        assert np.array_equal(run_gpu(xb, frames), want)
+        return
+    # promise: the first loads of a frame overlap the tail of the previous kernel of the stream; two integrations queued
+    dev = [torch.from_numpy(fr).cuda() for fr in frames]
+    x = xb.XCorr(n, f, t)
+    x.promise_complete_frames()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        for d in dev:
+            x.process(d, st)
+        first = x.read(None, st)
+        x.process(dev[1], st)
+        second = x.read(None, st)
+    torch.cuda.synchronize()
+    assert np.array_equal(first.cpu().numpy(), want)
+    assert np.array_equal(second.cpu().numpy(), oracle.planar(frames[1]))
+    x.close()
 
 
 def test_all_minus_eight_and_extremes(xb):
@@ -262,28 +329,43 @@ def _check_full_size(fr, got, n_samples=1500, n_probe=2, channels=None, seed=0):
             assert oracle.freivalds_lhs(tri, n, u, w) == oracle.freivalds_rhs(fch, u, w)
 
 
+def _channels(fr, chans):
+    """oracle.planar on the listed whole channels of a frame -> int32 [len(chans)][P][2]."""
+    return oracle.planar(np.ascontiguousarray(fr[:, list(chans), :]))
+
+
 def test_c2_full_size(xb):
     c = wl.CONFIGS["C2"]
     fr = c.frame()
     assert fr.nbytes == 268_435_456
+    smax, _ = segments_per_worker(xb, c.n_inputs, c.n_freq, c.n_time)
+    assert smax >= 2                      # every item is cut in time between two workers (64 items on 74 workers)
     got = run_gpu(xb, [fr])
     assert got.nbytes == 16_842_752
-    _check_full_size(fr, got, channels=range(0, 64, 3))
-    # whole matrix, every element: against the SIMT second opinion (held to the same oracle checks above)
-    ref = run_gpu(xb, [fr], simt=True)
-    assert np.array_equal(got, ref)
-    # two channels in full against the oracle
-    part = oracle.planar(fr, 17, 19)
-    assert np.array_equal(got[17:19], part[17:19])
+    # whole output, all 64 channels, every element, against the oracle
+    assert np.array_equal(got, oracle.planar(fr))
+    _check_full_size(fr, got, channels=range(0, 64, 7))
+    # the same with the promise bench.py runs under
+    assert np.array_equal(run_gpu(xb, [fr], promise=True), got)
+    # extra: the standalone SIMT second opinion agrees as well
+    assert np.array_equal(got, run_simt(fr))
 
 
 def test_c4_full_size(xb):
     c = wl.CONFIGS["C4"]
     fr = c.frame()
     got = run_gpu(xb, [fr])
-    _check_full_size(fr, got, n_samples=3000, channels=[0, 7, 15])
-    ref = run_gpu(xb, [fr], simt=True)
-    assert np.array_equal(got, ref)
+    # whole channels against the oracle: 0 and 7 from the data-parallel part of the schedule (items that run whole on one
+    # worker), 14 and 15 from the water-filled remainder (items cut in time, up to 9 segments per worker)
+    seg, wb = xb.xcorr_debug_schedule(c.n_inputs, c.n_freq, c.n_time, 74)
+    n_stage = -(-c.n_time // xb.xcorr_debug_stage_samples())
+    whole = {int(s[0]) for s in seg if s[4] - s[3] == n_stage}
+    cut = {int(s[0]) for s in seg if s[4] - s[3] < n_stage}
+    chans = [0, 7, 14, 15]
+    assert {0, 7} <= whole and {14, 15} & cut
+    assert np.array_equal(got[chans], _channels(fr, chans))
+    _check_full_size(fr, got, n_samples=3000, channels=[3, 11])
+    assert np.array_equal(got, run_simt(fr))             # extra: whole matrix against the SIMT second opinion
     # the common sky signal makes off-diagonal real parts positive on average (~2*T)
     off = got[0, 1:2048, 0].astype(np.float64)
     assert 1.0 < off.mean() / c.n_time < 3.0
@@ -307,35 +389,159 @@ def test_c5_full_size_stress(xb):
     for i in (0, 200):
         seg = got[3, oracle.pair_index(n, i, 256): oracle.pair_index(n, i, 511) + 1]
         assert np.array_equal(seg[:, 0], -8 * sr - 8 * si) and np.array_equal(seg[:, 1], 8 * si - 8 * sr)
-    _check_full_size(fr, got, n_samples=1200, channels=[0, 31], n_probe=1)
-    ref = run_gpu(xb, [fr], simt=True)
-    assert np.array_equal(got, ref)
+    # whole channels against the oracle: 0 (data-parallel part of the schedule), 24 and 31 (water-filled remainder)
+    chans = [0, 24, 31]
+    assert np.array_equal(got[chans], _channels(fr, chans))
+    _check_full_size(fr, got, n_samples=1200, channels=[12], n_probe=1)
+    assert np.array_equal(got, run_simt(fr))             # extra
 
 
-def test_c3_streamed_shape_reduced_frames(xb):
-    # C3's shape (N=256, F=1024, T=4096, 1 GiB frames) streamed from pinned memory; a pool of 2 distinct seeded
-    # frames is cycled 3 times (6 frames) -- by linearity the result must be 3 * (oracle(A) + oracle(B)).
+C3_POOL = 4   # distinct seeded 1 GiB frames, cycled 16 times = the 64 consecutive frames of BASELINE.json:configs[2]
+
+
+def test_c3_streamed_64_frames(xb):
+    """C3 as specified: N=256, F=1024, T=4096 (1 GiB frames), 64 frames streamed from pinned host memory through the
+    double-buffered H2D ring with the promise bench.py uses, ONE read at the end.  The 64 frames are a pool of C3_POOL = 4
+    distinct seeded frames cycled 16 times; by linearity the result must be 16 * sum_p oracle(frame_p)."""
     c = wl.CONFIGS["C3"]
-    pool = [torch.from_numpy(c.frame(k)).pin_memory() for k in range(2)]
+    assert c.n_frames == 64 and 64 % C3_POOL == 0
+    reps = c.n_frames // C3_POOL
+    pool = [torch.from_numpy(c.frame(k)).pin_memory() for k in range(C3_POOL)]
+    smax, smin = segments_per_worker(xb, c.n_inputs, c.n_freq, c.n_time)
+    assert smax >= 3 and smin >= 3
     x = xb.XCorr(c.n_inputs, c.n_freq, c.n_time)
+    x.promise_complete_frames()
     s = xb.XCorrStream(x, depth=2)
-    for rep in range(3):
-        for p in pool:
-            s.submit(p)
+    for k in range(c.n_frames):
+        s.submit(pool[k % C3_POOL])
     out = torch.empty((c.n_freq, x.n_pairs, 2), dtype=torch.int32).pin_memory()
     s.read(out)
     got = out.numpy()
     s.close()
     x.close()
-    chans = [0, 511, 1023]
-    want = sum(oracle.planar(np.ascontiguousarray(p.numpy()[:, chans, :])).astype(np.int64) for p in pool) * 3
+    # whole channels, element by element: first, last, and some in between (every worker's segment list is touched)
+    chans = [0, 1, 73, 74, 511, 1000, 1023]
+    want = sum(_channels(p.numpy(), chans).astype(np.int64) for p in pool) * reps
     assert np.array_equal(got[chans], want)
     rng = np.random.default_rng(5)
     idx = _sample_pairs(rng, 256, 1024, 1500)
-    want = 3 * sum(oracle.pairs(p.numpy(), idx) for p in pool)
+    want = reps * sum(oracle.pairs(p.numpy(), idx) for p in pool)
     pp = idx[:, 1].astype(np.int64) * (2 * 256 - idx[:, 1] + 1) // 2 + (idx[:, 2] - idx[:, 1])
     assert np.array_equal(got[idx[:, 0], pp].astype(np.int64), want)
-    # total-power identity on every 16th channel (linear in the frame, so it sums over the 6 frames too)
+    # total-power identity on every 16th channel (linear in the frame, so it sums over the 64 frames too)
     for ch in range(0, 1024, 16):
-        rhs = 3 * sum(int(oracle.identity_total_power(np.ascontiguousarray(p.numpy()[:, ch:ch + 1, :]))[0]) for p in pool)
+        rhs = reps * sum(int(oracle.identity_total_power(np.ascontiguousarray(p.numpy()[:, ch:ch + 1, :]))[0]) for p in pool)
         assert int(oracle.lhs_total_power(got[ch:ch + 1], 256)[0]) == rhs
+    # extra: the whole 269 MB result against the SIMT second opinion, frame by frame
+    ref = sum(run_simt(p.numpy()).astype(np.int64) for p in pool) * reps
+    assert np.array_equal(got, ref)
+
+
+# ------------------------------------------------------------------ streamed path with the promise (bench.py's e2e configuration)
+def test_streamed_path_with_promise_distinct_frames_per_slot(xb):
+    """xcorr_stream_submit + read_async, depth 2, promise on, 7 distinct frames (so each ring slot is rewritten with new
+    data several times while the previous kernel may still be draining) -- shapes with several segments per worker."""
+    for (n, f, t) in [(256, 160, 192), (512, 60, 192)]:
+        frames = [wl.gaussian_frame(n, f, t, seed=7000 + n + k) for k in range(7)]
+        pinned = [torch.from_numpy(fr).pin_memory() for fr in frames]
+        x = xb.XCorr(n, f, t)
+        x.promise_complete_frames()
+        s = xb.XCorrStream(x, depth=2)
+        outs = [torch.empty((f, x.n_pairs, 2), dtype=torch.int32).pin_memory() for _ in frames]
+        for p_, o in zip(pinned, outs):          # one integration per frame, nothing waits in between
+            s.submit(p_)
+            s.read_async(o)
+        s.sync()
+        for fr, o in zip(frames, outs):
+            assert np.array_equal(o.numpy(), oracle.planar(fr))
+        for p_ in pinned:                        # and all seven into one integration
+            s.submit(p_)
+        out = torch.empty((f, x.n_pairs, 2), dtype=torch.int32).pin_memory()
+        s.read(out)
+        assert np.array_equal(out.numpy(), sum(oracle.planar(fr).astype(np.int64) for fr in frames))
+        s.close()
+        x.close()
+
+
+# ------------------------------------------------------------------ handle state across streams
+def test_process_and_read_on_different_streams_are_ordered(xb):
+    """include/xcorr.h: a call on another stream than the handle's previous call waits, on the device, for that call's work."""
+    n, f, t = 256, 160, 192
+    frames = [wl.uniform_frame(n, f, t, seed=8100 + k) for k in range(3)]
+    dev = [torch.from_numpy(fr).cuda() for fr in frames]
+    torch.cuda.synchronize()
+    x = xb.XCorr(n, f, t)
+    sa, sb, sc = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    for rep in range(4):
+        x.process(dev[0], sa)
+        x.process(dev[1], sb)        # another stream: must see frame 0's slots
+        outs.append(x.read(None, sc))  # a third one: must see both
+        x.process(dev[2], sa)        # next integration, back on the first stream: must not overtake the read
+        outs.append(x.read(None, sb))
+    torch.cuda.synchronize()
+    want01 = oracle.planar(frames[0]).astype(np.int64) + oracle.planar(frames[1])
+    want2 = oracle.planar(frames[2])
+    for k, o in enumerate(outs):
+        assert np.array_equal(o.cpu().numpy(), want01 if k % 2 == 0 else want2), k
+    x.close()
+
+
+# ------------------------------------------------------------------ modulo-2^32 behaviour of the offset sums inside a slot
+def test_offset_sums_wrap_inside_tmem_and_inside_a_slot(xb):
+    """The tensor core is fed offset operands, so the sums held in TMEM and in an accumulator slot grow far
+    faster than the visibilities (up to 900 per sample against 128) and wrap modulo 2^32 long before the int32 guard
+    (16,777,215 samples).  F = n_workers channels of N = 16: every item runs whole on one worker, so ONE TMEM accumulator
+    integrates all T = 5,000,000 samples of a frame (wraps in TMEM), and three frames are reduce-added into the same slot
+    (wraps in cp.reduce.async.bulk .add.s32).  Closed form per pair."""
+    w = n_workers()
+    n, f, t = 16, w, 5_000_000
+    seg, wb = xb.xcorr_debug_schedule(n, f, t, w)
+    assert len(seg) == f and (np.diff(wb) == 1).all()            # one whole item per worker
+    fr = torch.empty((t, f, n), dtype=torch.uint8, device="cuda")
+    fr[:, :, 0::2] = 0x77        #  7 + 7i  -> offset operands 15, 15 (largest products)
+    fr[:, :, 1::2] = 0x87        # -8 + 7i
+    x = xb.XCorr(n, f, t)
+    for _ in range(3):
+        x.process(fr.reshape(-1))
+    got = x.read().cpu().numpy().astype(np.int64)
+    x.close()
+    vals = {0: 7 + 7j, 1: -8 + 7j}
+    want = np.zeros((n * (n + 1) // 2, 2), dtype=np.int64)
+    for i in range(n):
+        for j in range(i, n):
+            v = vals[i % 2] * np.conj(vals[j % 2]) * (3 * t)
+            want[oracle.pair_index(n, i, j)] = (int(v.real), int(v.imag))
+    assert np.array_equal(got, np.broadcast_to(want, got.shape))
+
+
+# ------------------------------------------------------------------ NEXT-3: several handles on disjoint channel ranges (PAPER.md:51, :111)
+@pytest.mark.parametrize("split", ["two_ranks", "streams_3_3_2"])
+def test_channel_range_replicas_through_the_c_abi(xb, split):
+    """Each GPU of a server correlates its own streams' channels; the merged result is the concatenation along f
+    (PAPER.md:51 "each of the AMD R9 280X GPUs processes 3 of these streams, and the R9 270X processes 2"; :111 "combines
+    all eight streams").  Here: one handle per channel range on one GPU, each fed its slice of the frame."""
+    from paper_1503_06189_b200 import replicas
+    n, f, t = 256, 64, 320
+    if split == "two_ranks":
+        ranges = replicas.channel_ranges(f, 2)
+    else:
+        ranges, b = [], 0
+        for n_streams in (3, 3, 2):                          # 8 streams of 8 channels
+            ranges.append((b, b + 8 * n_streams))
+            b += 8 * n_streams
+        assert b == f
+    frames = [wl.gaussian_frame(n, f, t, seed=8200 + k) for k in range(2)]
+    handles = [xb.XCorr(n, e - b, t) for b, e in ranges]
+    streams = [torch.cuda.Stream() for _ in ranges]
+    for fr in frames:
+        for (b, e), x, st in zip(ranges, handles, streams):
+            with torch.cuda.stream(st):
+                x.process(torch.from_numpy(np.ascontiguousarray(fr[:, b:e, :])).cuda(), st)
+    parts = [x.read(None, st) for x, st in zip(handles, streams)]
+    torch.cuda.synchronize()
+    merged = np.concatenate([p.cpu().numpy() for p in parts], axis=0)
+    want = sum(oracle.planar(fr).astype(np.int64) for fr in frames)
+    assert np.array_equal(merged, want)
+    for x in handles:
+        x.close()
