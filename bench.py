@@ -2,6 +2,7 @@
 """bench.py -- X-engine throughput on synthetic CHIME-shaped frames (BASELINE.json metric), one JSON line.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2|C4|C5|C3] [--impl reference]
+                    [--no-sustained] [--no-other-configs] [--no-e2e] [--no-next-rows] [--no-cpu-baseline] [--no-int8-probe]
 
 A "step" is one pass of the whole hot path over one frame: xcorr_process (TMA stage -> nibble unpack -> tcgen05
 int8 MMAs -> epilogue, rows a1..a4) followed by xcorr_read (the packed-triangle epilogue that ends the integration;
@@ -9,6 +10,11 @@ BASELINE.json:configs[1] "one integration per frame").  `value` is input Gb/s wi
 HBM; `e2e` is the same metric through the streamed C-ABI path (row a5) with page-locked HOST frames and a HOST
 result, copies inside the timed region.  Inputs are synthetic (workloads.py) and larger than L2 (256 MiB frames,
 two of them alternating), so no flush is needed between iterations.
+
+Beside the K timed steps the line carries a `sustained` leg (the same step back to back for >= 2 s with the clocks sampled
+during that leg only: the power-capped steady state), `other_configs` (C3: the 64-frame streamed run of BASELINE.json
+configs[2] in Gb/s with its H2D-only ceiling; C4, C5: step and kernel times, useful and issued int8 TOP/s) and the
+measured int8 issue ceiling of the tensor pipe (paper_1503_06189_b200/probe.py) as roofline.int8_issue_ceiling_tops.
 
 Multi-GPU: the path does not shard ("replicas only"): --gpus N (under torchrun) runs N independent
 replicas, one per GPU, no collective on the data path; value = N frames' bits / max-over-ranks time.
@@ -36,6 +42,14 @@ NOMINAL_INT8_TOPS = 4500.0  # dense int8, B200 nominal (2x the 2.25 PFLOP/s dens
 # dram__bytes_read.sum + dram__bytes_write.sum of xengine_kernel<false> for one C2 launch, from the committed
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
 NCU_TRAFFIC_BYTES = {"C2": 277.2e6}   # profiles/r01_ncu_full_bench_c2.md: 268.49 MB read + 8.66 MB written
+# tcgen05 MMAs (M256 N256 K32, 2 CTAs) xengine_kernel issues per 32-sample K-step of a 256 x 256 super-tile
+MMAS_DIAG, MMAS_OFFDIAG = 3, 4
+
+
+def issued_over_useful(cfg) -> float:
+    """int8 ops the kernel issues / useful ops (8 per complex MAC, pairs i <= j only)."""
+    nb = -(-cfg.n_inputs // 256)
+    return (MMAS_DIAG * nb + MMAS_OFFDIAG * nb * (nb - 1) // 2) * 65536 / (4.0 * cfg.n_pairs)
 
 
 def load_peaks():
@@ -219,6 +233,135 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+class Resident:
+    """One config with its frames resident in HBM: handle, two distinct device frames, output buffer, stream."""
+
+    def __init__(self, cfg, xb, torch, n_distinct=2):
+        self.cfg, self.torch = cfg, torch
+        self.host_frames = [cfg.frame(k) for k in range(n_distinct)]
+        self.dev_frames = [torch.from_numpy(f).cuda() for f in self.host_frames]
+        self.x = xb.XCorr(cfg.n_inputs, cfg.n_freq, cfg.n_time)
+        self.x.promise_complete_frames()      # the frames are resident and complete long before any launch (include/xcorr.h)
+        self.out_dev = torch.empty((cfg.n_freq, cfg.n_pairs, 2), dtype=torch.int32, device="cuda")
+        self.st = torch.cuda.Stream()
+        self.n_distinct = n_distinct
+
+    def step(self, k):
+        self.x.process(self.dev_frames[k % self.n_distinct], self.st)
+        self.x.read(self.out_dev, self.st)
+
+    def timed_steps(self, steps, barrier):
+        """K whole steps between two CUDA events on the launching stream -> total ms."""
+        torch = self.torch
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(self.st)
+        for k in range(steps):
+            self.step(k)
+        e1.record(self.st)
+        barrier()
+        return e0.elapsed_time(e1)
+
+    def timed_kernels(self, steps, barrier):
+        """The same loop with events around every xcorr_process -> list of xengine_kernel durations in ms."""
+        torch = self.torch
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for k in range(steps):
+            evs[k][0].record(self.st)
+            self.x.process(self.dev_frames[k % self.n_distinct], self.st)
+            evs[k][1].record(self.st)
+            self.x.read(self.out_dev, self.st)
+        barrier()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    def close(self):
+        self.x.close()
+        self.dev_frames = self.host_frames = None
+
+
+def tensor_roofline(cfg, k_ms, peaks, ceiling=None):
+    """Tensor roofline entries of xengine_kernel for one launch of `cfg` taking k_ms."""
+    alg_ops = 8.0 * cfg.cmacs_per_frame              # 4 real MACs = 8 int8 ops per complex MAC, useful pairs i<=j only
+    achieved = alg_ops / (k_ms * 1e-3) / 1e12
+    peak = 2.0 * peaks["bf16_burst"]
+    peak_sustained = 2.0 * peaks["bf16_sustained"] if peaks.get("bf16_sustained") else None
+    iou = issued_over_useful(cfg)
+    r = {"bound": "tensor", "kernel": "xengine_kernel (xcorr_process)", "achieved": achieved, "peak": peak, "unit": "TOP/s",
+         "frac": achieved / peak, "kernel_ms": k_ms, "algorithmic_ops_per_launch": alg_ops,
+         "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
+         "frac_of_sustained_peak": (achieved / peak_sustained) if peak_sustained else None, "peak_sustained": peak_sustained,
+         "issued_over_useful": iou, "issued_int8_tops": achieved * iou,
+         "hbm_gbs_staging": cfg.frame_bytes / (k_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]}
+    if ceiling:
+        r["int8_issue_ceiling_tops"] = ceiling["burst_tops"]
+        r["frac_useful_of_issue_ceiling"] = achieved / ceiling["burst_tops"]
+        r["frac_issued_of_issue_ceiling"] = achieved * iou / ceiling["burst_tops"]
+    return r
+
+
+def measure_other_config(name, xb, torch, peaks, ceiling, steps=20):
+    """C4 / C5 (device-resident step) and C3 (device-resident step + the 64-frame streamed run of BASELINE.json configs[2])."""
+    cfg = wl.CONFIGS[name]
+    r = Resident(cfg, xb, torch)
+
+    def barrier():
+        torch.cuda.synchronize()
+
+    for k in range(3):
+        r.step(k)
+    total_ms = r.timed_steps(steps, barrier)
+    kern = r.timed_kernels(steps, barrier)
+    k_ms = statistics.mean(kern)
+    ms = total_ms / steps
+    out = {"workload": name, "n_inputs": cfg.n_inputs, "n_freq": cfg.n_freq, "t_per_frame": cfg.n_time, "steps": steps,
+           "ms_per_step": ms, "value_gbps": 8.0 * cfg.frame_bytes / (ms * 1e-3) / 1e9, "cmac_per_s": cfg.cmacs_per_frame / (ms * 1e-3),
+           "kernel_ms": k_ms, "kernel_ms_min": min(kern), "roofline": tensor_roofline(cfg, k_ms, peaks, ceiling)}
+    if cfg.n_frames > 1:
+        # frames ADDED to a running integration (the streamed case: no read between frames), device resident
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r.x.read(r.out_dev, r.st)
+        barrier()
+        e0.record(r.st)
+        for k in range(steps):
+            r.x.process(r.dev_frames[k % 2], r.st)
+        e1.record(r.st)
+        barrier()
+        r.x.read(r.out_dev, r.st)
+        out["added_frame_kernel_ms"] = e0.elapsed_time(e1) / steps
+        # BASELINE.json configs[2]: n_frames consecutive frames from pinned host memory, double-buffered H2D overlapped with
+        # the correlation, ONE read at the end
+        pinned = [torch.from_numpy(f).pin_memory() for f in r.host_frames]
+        out_host = torch.empty((cfg.n_freq, cfg.n_pairs, 2), dtype=torch.int32).pin_memory()
+        s = xb.XCorrStream(r.x, depth=2)
+        for k in range(2):
+            s.submit(pinned[k % 2])
+        s.read(out_host)
+        barrier()
+        t0 = time.perf_counter()
+        for k in range(cfg.n_frames):
+            s.submit(pinned[k % 2])
+        s.read(out_host)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        hb = torch.empty(cfg.frame_bytes, dtype=torch.uint8, device="cuda")
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        for k in range(4):
+            hb.copy_(pinned[k % 2].view(-1), non_blocking=True)
+        torch.cuda.synchronize()
+        h2d = 8.0 * 4 * cfg.frame_bytes / (time.perf_counter() - t1) / 1e9
+        del hb
+        s.close()
+        out["streamed"] = {"value": 8.0 * cfg.frame_bytes * cfg.n_frames / dt / 1e9, "unit": "Gb/s", "frames": cfg.n_frames,
+                           "pool": 2, "ms_per_frame": dt / cfg.n_frames * 1e3, "h2d_only_gbps": h2d, "paper_rate_gbps": 819.2,
+                           "h2d_bytes_per_frame": cfg.frame_bytes, "d2h_bytes_total": cfg.output_bytes,
+                           "api": f"{cfg.n_frames} x xcorr_stream_submit(pinned host frame, pool of 2 distinct frames cycled) + one "
+                                  "xcorr_stream_read(pinned host out); host wall clock from the first submit to the result in host memory"}
+    r.close()
+    torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -230,6 +373,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-next-rows", action="store_true")
     ap.add_argument("--no-int8-probe", action="store_true")
+    ap.add_argument("--no-sustained", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true")
+    ap.add_argument("--sustained-seconds", type=float, default=2.0)
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
     if args.impl == "reference":
@@ -237,7 +383,7 @@ def main():
 
     import torch
     import paper_1503_06189_b200 as xb
-    from paper_1503_06189_b200 import replicas
+    from paper_1503_06189_b200 import probe, replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -252,19 +398,12 @@ def main():
     warm = max(3, args.warmup)
     steps = max(1, args.steps)
     peaks = load_peaks()
+    solo = rank == 0 and world == 1
 
     # ---- synthetic inputs, resident in HBM before the timed region: two distinct frames, alternating
     n_distinct = 2
-    host_frames = [cfg.frame(k) for k in range(n_distinct)]
-    dev_frames = [torch.from_numpy(f).cuda() for f in host_frames]
-    x = xb.XCorr(cfg.n_inputs, cfg.n_freq, cfg.n_time)
-    x.promise_complete_frames()      # the frames are resident and complete long before any launch (include/xcorr.h)
-    out_dev = torch.empty((cfg.n_freq, cfg.n_pairs, 2), dtype=torch.int32, device="cuda")
-    st = torch.cuda.Stream()
-
-    def step(k):
-        x.process(dev_frames[k % n_distinct], st)
-        x.read(out_dev, st)
+    r = Resident(cfg, xb, torch, n_distinct)
+    x, st, host_frames = r.x, r.st, r.host_frames
 
     def barrier():
         torch.cuda.synchronize()
@@ -273,31 +412,17 @@ def main():
         torch.cuda.synchronize()
 
     for k in range(warm):
-        step(k)
+        r.step(k)
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.15)
     # -- timed region 1: K whole steps, CUDA events on the launching stream
     launches0 = x.kernel_launches
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record(st)
-    for k in range(steps):
-        step(k)
-    e1.record(st)
-    barrier()
-    total_ms = e0.elapsed_time(e1)
+    total_ms = r.timed_steps(steps, barrier)
     launches = x.kernel_launches - launches0
     # -- timed region 2 (same loop, per-kernel events): duration of the dominant kernel (xengine_kernel = xcorr_process)
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-    for k in range(steps):
-        evs[k][0].record(st)
-        x.process(dev_frames[k % n_distinct], st)
-        evs[k][1].record(st)
-        x.read(out_dev, st)
-    barrier()
-    kern_ms = [a.elapsed_time(b) for a, b in evs]
+    kern_ms = r.timed_kernels(steps, barrier)
     clocks = sampler.stop()
 
     total_ms = replicas.max_over_ranks(total_ms, dist, "cuda")
@@ -306,27 +431,29 @@ def main():
     value = world * bits_per_frame / (ms_per_step * 1e-3) / 1e9
     cmac_per_s = world * cfg.cmacs_per_frame / (ms_per_step * 1e-3)
 
+    # ---- the int8 tensor issue ceiling of this box (resident operands, no TMA / unpack / epilogue): burst and >= 4 s sustained
+    ceiling = None
+    if rank == 0 and not args.no_int8_probe:
+        try:
+            ceiling = probe.int8_issue_ceiling(pattern=1, sustained_seconds=4.0 if solo else 1.0)
+        except Exception as e:
+            ceiling = None
+            probe_error = str(e)[:160]
+
     # ---- roofline of the dominant kernel (tensor-bound: a dense int8 contraction)
     k_ms = statistics.mean(kern_ms)
-    alg_ops = 8.0 * cfg.cmacs_per_frame              # 4 real MACs = 8 int8 ops per complex MAC, useful pairs i<=j only
-    achieved = alg_ops / (k_ms * 1e-3) / 1e12
-    # int8 = 2 x bf16 (nominal ratio 4.5 : 2.25) x the measured bf16 figure.  The burst figure is used whatever the length
-    # of the timed region (the larger denominator, so the smaller fraction); the fraction of the sustained figure is
-    # reported beside it because a default run (2000 back-to-back steps) is long enough to be power-capped.
-    peak = 2.0 * peaks["bf16_burst"]
-    peak_sustained = 2.0 * peaks["bf16_sustained"] if peaks.get("bf16_sustained") else None
-    roofline = {
-        "bound": "tensor", "kernel": "xengine_kernel (xcorr_process)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-        "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
-        "peak_source": f"2 x bf16_tflops (burst) of MEASURED_PEAKS.json [{peaks['source']}]; int8:bf16 nominal ratio 4.5:2.25",
-        "kernel_ms": k_ms, "kernel_ms_min": min(kern_ms), "algorithmic_ops_per_launch": alg_ops,
-        "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
-        "frac_of_sustained_peak": (achieved / peak_sustained) if peak_sustained else None, "peak_sustained": peak_sustained,
-        "hbm_gbs_staging": cfg.frame_bytes / (k_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"],
-    }
+    # `frac` keeps the 2 x measured bf16 burst peak as denominator (int8:bf16 nominal ratio 4.5:2.25) for continuity; the
+    # measured issue ceiling of the int8 pipe itself is beside it (int8_issue_ceiling_tops, frac_*_of_issue_ceiling)
+    roofline = tensor_roofline(cfg, k_ms, peaks, ceiling)
+    roofline["traffic"] = NCU_TRAFFIC_BYTES.get(cfg.name)
+    roofline["kernel_ms_min"] = min(kern_ms)
+    roofline["peak_source"] = f"2 x bf16_tflops (burst) of MEASURED_PEAKS.json [{peaks['source']}]; int8:bf16 nominal ratio 4.5:2.25"
+    if ceiling:
+        roofline["int8_issue_ceiling"] = ceiling
+    elif rank == 0 and not args.no_int8_probe:
+        roofline["int8_issue_ceiling_error"] = probe_error
 
-    # context for the denominator: the library's own int8 GEMM on this box in this run (cuBLAS through torch._int_mm,
-    # 8192^3, best of 10 after 3 warm-ups).  Not used for `frac`; shows where a plain int8 contraction lands on this part.
+    # context: the library's own int8 GEMM on this box in this run (cuBLAS through torch._int_mm, 8192^3, best of 10)
     if rank == 0 and not args.no_int8_probe:
         try:
             ga = torch.randint(-8, 8, (8192, 8192), dtype=torch.int8, device="cuda")
@@ -341,14 +468,38 @@ def main():
                 if k >= 3:
                     best = g0.elapsed_time(g1) if best is None else min(best, g0.elapsed_time(g1))
             roofline["cublas_int8_gemm_8192_tops_burst"] = 2.0 * 8192 ** 3 / (best * 1e-3) / 1e12
-            nb = -(-cfg.n_inputs // 256)                       # 256 x 256 super-tiles: 3 MMAs on the diagonal, 4 above it
-            issued_over_useful = (3 * nb + 4 * nb * (nb - 1) // 2) * 65536 / (4.0 * cfg.n_pairs)
-            roofline["issued_over_useful"] = issued_over_useful
-            roofline["issued_int8_tops"] = achieved * issued_over_useful
             del ga, gb
         except Exception as e:  # the probe is context only
             roofline["cublas_int8_gemm_8192_tops_burst"] = None
             roofline["int8_probe_error"] = str(e)[:120]
+
+    # ---- sustained leg: the same step back to back for >= sustained_seconds, clocks sampled during this leg only
+    sustained = None
+    if not args.no_sustained:
+        n_sus = max(steps, int(args.sustained_seconds * 1e3 / ms_per_step))
+        n_ker = max(20, n_sus // 4)
+        for k in range(n_sus // 4):                       # bring the part to its steady state first (not timed)
+            r.step(k)
+        barrier()
+        sus_sampler = ClockSampler(local)
+        sus_sampler.start()
+        sus_total = r.timed_steps(n_sus, barrier)
+        sus_kern = r.timed_kernels(n_ker, barrier)
+        sus_clocks = sus_sampler.stop()
+        sus_total = replicas.max_over_ranks(sus_total, dist, "cuda")
+        sus_ms = sus_total / n_sus
+        sus_k = statistics.mean(sus_kern)
+        sus_ach = 8.0 * cfg.cmacs_per_frame / (sus_k * 1e-3) / 1e12
+        sustained = {"steps": n_sus, "seconds": sus_total * 1e-3, "ms_per_step": sus_ms,
+                     "value": world * bits_per_frame / (sus_ms * 1e-3) / 1e9, "unit": "Gb/s",
+                     "cmac_per_s": world * cfg.cmacs_per_frame / (sus_ms * 1e-3),
+                     "kernel_ms": sus_k, "kernel_steps": n_ker, "useful_int8_tops": sus_ach,
+                     "frac_of_2x_bf16_sustained": sus_ach / (2.0 * peaks["bf16_sustained"]) if peaks.get("bf16_sustained") else None,
+                     "frac_of_2x_bf16_burst": sus_ach / (2.0 * peaks["bf16_burst"]),
+                     "frac_of_nominal_4500": sus_ach / NOMINAL_INT8_TOPS,
+                     "step_pct_of_nominal_4500": 100.0 * 8.0 * cfg.cmacs_per_frame / (sus_ms * 1e-3) / (NOMINAL_INT8_TOPS * 1e12),
+                     "frac_useful_of_issue_ceiling_sustained": (sus_ach / ceiling["sustained_tops"]) if ceiling else None,
+                     "clocks": sus_clocks}
 
     # ---- e2e: streamed C-ABI path, HOST frames in, HOST visibilities out, every step
     e2e = None
@@ -400,18 +551,34 @@ def main():
                "d2h_bytes_per_step": d2h, "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3, "api": api,
                "h2d_only_gbps": h2d_gbps, "paper_rate_gbps": 819.2 if cfg.name == "C3" else None}
         s.close()
+        del pinned
 
     # ---- the rows SURVEY.md 8(f) marks "next", same frame shape, timed one by one with CUDA events (not part of `value`)
     next_rows = None
-    if rank == 0 and world == 1 and not args.no_next_rows and cfg.n_freq % wl.PACKET_F == 0 and cfg.n_time % wl.PACKET_T == 0:
+    if solo and not args.no_next_rows and cfg.n_freq % wl.PACKET_F == 0 and cfg.n_time % wl.PACKET_T == 0:
         next_rows = measure_next_rows(cfg, x, xb, torch, st, host_frames[0], peaks)
+    r.close()
+    torch.cuda.empty_cache()
+
+    # ---- the other BASELINE.json configs, a few steps each (inputs generated outside the timed regions)
+    other = None
+    if solo and not args.no_other_configs:
+        other = {}
+        for name in ("C3", "C4", "C5"):
+            if name == cfg.name:
+                continue
+            try:
+                other[name] = measure_other_config(name, xb, torch, peaks, ceiling)
+            except Exception as e:      # e.g. not enough pinned host memory for C3 on a small box: say so, keep the line
+                other[name] = {"error": str(e)[:200]}
 
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if solo and not args.no_cpu_baseline:
         cpu = oracle_sample(cfg)
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "cmac_per_s")}
 
     if rank == 0:
+        peak = roofline["peak"]
         line = {
             "metric": "xengine_input_gbps", "value": value, "unit": "Gb/s", "n_gpus": world, "steps": steps, "warmup": warm,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8",
@@ -424,10 +591,10 @@ def main():
             "pct_int8_peak_nominal": 100.0 * 8.0 * cmac_per_s / world / (NOMINAL_INT8_TOPS * 1e12),
             "pct_int8_peak_measured": 100.0 * 8.0 * cmac_per_s / world / (peak * 1e12),
             "paper_context": "51.2 Gb/s per 3-GPU server, 819.2 Gb/s over 16 servers (PAPER.md Table I; other hardware)",
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "next_rows": next_rows, "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": roofline, "sustained": sustained, "cpu_baseline": cpu, "e2e": e2e, "other_configs": other,
+            "next_rows": next_rows, "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
-    x.close()
     if dist is not None:
         dist.destroy_process_group()
 
