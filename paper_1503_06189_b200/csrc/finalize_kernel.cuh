@@ -8,10 +8,13 @@
 // h = h' - 8, l = l' - 8, the column sums sh_n = sum_t h'_n, sl_n = sum_t l'_n of the tile's sum slots and
 // T' = the number of (zero-padded) samples the tensor path has integrated,
 //
-//   Re V[i,j] = R'[i,j] - 8 (sh_i + sl_i + sh_j + sl_j) + 128 T'
-//   Im V[i,j] = Q'[i,j] - Q'[j,i] + 8 (sh_i - sl_i) - 8 (sh_j - sl_j)               on diagonal super-tiles (I == J)
-//   Im V[i,j] = Q'[i,j] - 7 sh_i - 8 sl_i - 8 sh_j + 8 sl_j                         for I < J, where Q' holds
-//               sum l'_i h'_j + h'_i (15 - l'_j)
+//   I < J (R' = sum h'_i h'_j + l'_i l'_j,  Q' = sum l'_i h'_j + h'_i (15 - l'_j)):
+//     Re V[i,j] = R'[i,j] - 8 (sh_i + sl_i + sh_j + sl_j) + 128 T'
+//     Im V[i,j] = Q'[i,j] - 7 sh_i - 8 sl_i - 8 sh_j + 8 sl_j
+//   I == J (R' = G' = sum (h'_i + l'_i)(h'_j + l'_j),  Q' = X' = sum l'_i h'_j; xengine_kernel.cuh header):
+//     G = G' - 16 (sh_i + sl_i + sh_j + sl_j) + 256 T',   X[i,j] = X'[i,j] - 8 sl_i - 8 sh_j + 64 T',   hence
+//     Re V[i,j] = G - X[i,j] - X[j,i] = G'[i,j] - X'[i,j] - X'[j,i] - 8 (sh_i + sl_i + sh_j + sl_j) + 128 T'
+//     Im V[i,j] = X[i,j] - X[j,i]     = X'[i,j] - X'[j,i] + 8 (sh_i - sl_i) - 8 (sh_j - sl_j)
 //
 // exactly, modulo 2^32 (unsigned arithmetic below; the true values fit int32 by the overflow guard).
 #pragma once
@@ -117,10 +120,14 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
         const int i = i0 + ic, j = j0 + tx;
         if (j < n_inputs && i <= j) {
             const uint32_t shi = sS[0][ic], sli = sS[1][ic];
-            const uint32_t re = sR[tx][ic] - 8u * (shi + sli + shj + slj) + 128u * offset_samples;
+            uint32_t re = sR[tx][ic] - 8u * (shi + sli + shj + slj) + 128u * offset_samples;
             uint32_t im;
-            if (diag_super) im = (i == j) ? 0u : sQ[tx][ic] - sX[tx][ic] + 8u * (shi - sli) - 8u * (shj - slj);
-            else im = sQ[tx][ic] - 7u * shi - 8u * sli - 8u * shj + 8u * slj;
+            if (diag_super) {
+                re -= sQ[tx][ic] + sX[tx][ic];
+                im = (i == j) ? 0u : sQ[tx][ic] - sX[tx][ic] + 8u * (shi - sli) - 8u * (shj - slj);
+            } else {
+                im = sQ[tx][ic] - 7u * shi - 8u * sli - 8u * shj + 8u * slj;
+            }
             const long long p = (long long)f * P + pair_index(n_inputs, i, j);
             if constexpr (kNormalise) {
                 // L = lost + c_i + c_j - X_ij (the point (i, i) receives its counter once); V~ = V * T / (T - L)

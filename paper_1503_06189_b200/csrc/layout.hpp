@@ -15,10 +15,12 @@
 // the epilogue stages in shared memory and hands to ONE bulk copy (first frame) or bulk int32 reduce-add (later frames).
 //
 //     row          = TMEM lane       : input  i = 256*I + 128*r + row
-//     col in [0,256)  "R" columns    : input  j = 256*J + col          value  Re V[i,j] = sum h_i h_j + l_i l_j
+//     col in [0,256)  "R" columns    : input  j = 256*J + col
+//         I <  J :  value  Re V[i,j] = sum h_i h_j + l_i l_j
+//         I == J :  value  G[i,j]    = sum (h_i + l_i)(h_j + l_j)
 //     col in [256,512) "Q" columns   : input  j = 256*J + (col-256)
 //         I <  J :  value  Im V[i,j] = sum l_i h_j - h_i l_j
-//         I == J :  value  X[i,j]    = sum l_i h_j ;   Im V[i,j] = X[i,j] - X[j,i]  is formed by xcorr_read
+//         I == J :  value  X[i,j]    = sum l_i h_j ;   Re V = G - X - X^T,  Im V = X - X^T  are formed by xcorr_read
 //
 // Lower-triangle R entries of diagonal super-tiles and anything with i >= N or j >= N are never read
 // (and mostly never written).
@@ -27,7 +29,8 @@
 // 15 - l' where a negated operand is needed) instead of the sign-extended int8 value: the upper nibble of every
 // operand byte is then constant zero, which measurably lowers the switching power of the MMA datapath (the part is
 // power-limited).  The slots therefore hold the OFFSET sums
-//     R'[i,j] = sum h'_i h'_j + l'_i l'_j          Q'[i,j] = sum l'_i h'_j  ( + h'_i (15 - l'_j) for I < J )
+//     I <  J :  R'[i,j] = sum h'_i h'_j + l'_i l'_j          Q'[i,j] = sum l'_i h'_j + h'_i (15 - l'_j)
+//     I == J :  R'[i,j] = sum (h'_i + l'_i)(h'_j + l'_j)      Q'[i,j] = sum l'_i h'_j
 // and every segment also owns a row of per-input column sums over its time range ("sum slot"):
 //
 //   sums[slot][r][plane][row]   int32,  plane 0: sum_t h'   1: sum_t l'   of input 256*I + 128*r + row   (A block)

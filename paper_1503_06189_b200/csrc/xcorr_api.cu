@@ -542,6 +542,8 @@ extern "C" void xcorr_stream_destroy(xcorr_stream *s)
     if (!s) return;
     if (s->h) cudaSetDevice(s->h->device);
     cudaDeviceSynchronize();
+    // everything the handle enqueued has finished, and the compute stream is about to go: nothing left to order after
+    if (s->h && s->h->has_last_stream && s->h->last_stream == s->compute_stream) s->h->has_last_stream = false;
     for (int k = 0; k < s->depth; ++k) {
         if (s->buf[k]) cudaFree(s->buf[k]);
         if (s->pkt_buf[k]) cudaFree(s->pkt_buf[k]);

@@ -12,9 +12,14 @@
 //   a4  epilogue warps tcgen05.ld the accumulators, stage them in shared memory and bulk-copy (first frame) or bulk
 //       reduce-add (later frames) them into this segment's accumulator slot
 //
-// Complex product from stacked real GEMMs (BASELINE.json:north_star (b)); h = Re plane, l = Im plane (offset values):
-//   diagonal super-tile (I == J):   R += h h^T ; R += l l^T ; Q += l h^T      (Im V = Q - Q^T, formed at read)
-//   off-diagonal        (I <  J):   R += h_I h_J^T ; R += l_I l_J^T ; Q += l_I h_J^T ; Q += h_I (15 - l_J)^T
+// Complex product from real GEMMs (BASELINE.json:north_star (b)); h = Re plane, l = Im plane, s = h + l (offset values):
+//   off-diagonal        (I <  J):   R += h_I h_J^T ; R += l_I l_J^T ; Q += l_I h_J^T ; Q += h_I (15 - l_J)^T     (4 MMAs per K-step)
+//   diagonal super-tile (I == J):   R += s s^T ; Q += l h^T                                                     (2 MMAs per K-step)
+// On the diagonal the tile is Hermitian, which lets three real products per complex MAC do (Gauss), two of them being the
+// two triangles of ONE full product:  with G = (h+l)(h+l)^T = hh^T + ll^T + hl^T + lh^T (symmetric) and X = l h^T,
+//     Re V[i,j] = G[i,j] - X[i,j] - X[j,i]        Im V[i,j] = X[i,j] - X[j,i]        (formed by xcorr_read, exact, no division)
+// so a diagonal super-tile costs 2 x 256 x 256 MACs per sample where the stacked form (hh^T, ll^T, lh^T) costs 3 -- at
+// N = 256 (every tile is diagonal) the kernel issues 0.996 of the "useful" 4 real MACs per complex pair i <= j.
 // Integer MMAs have no operand-negate bit, hence the explicit complement plane 15 - l'_J for I < J (the constant
 // 15 sum h'_I it adds is removed at read together with the offsets).
 //
@@ -39,10 +44,10 @@ struct KernelCfg {
     static constexpr int kRowBytes = 128;                          // one t-row of one 128-input block
     static constexpr int kPlaneBytes = kStageT * kRowBytes;        // 8 KiB: one plane (or packed block) per stage
     static constexpr int kPackedBlocks = kOffDiag ? 2 : 1;         // A block (+ B block when I < J)
-    static constexpr int kPlanes = kOffDiag ? 5 : 2;               // h_a l_a [h_b l_b 15-l_b]
+    static constexpr int kPlanes = kOffDiag ? 5 : 3;               // h_a l_a s_a   or   h_a l_a {s_a | h_b} l_b 15-l_b
     static constexpr int kPackedStageBytes = kPackedBlocks * kPlaneBytes;
     static constexpr int kPlaneStageBytes = kPlanes * kPlaneBytes;
-    static constexpr int kPackedStages = kOffDiag ? 3 : 4;
+    static constexpr int kPackedStages = 4;
     static constexpr int kPlaneStages = kOffDiag ? 3 : 6;
     static constexpr int kUnpackWarps = 8;                         // multiple of 4
     static constexpr int kUnpackThreads = kUnpackWarps * 32;
@@ -54,13 +59,30 @@ struct KernelCfg {
     static constexpr int kEpiStaging = 4 * 2 * kEpiStageBytes;     // 4 epilogue warps x 2 buffers (32 KiB)
     static constexpr int kSmemData = kPackedStages * kPackedStageBytes + kPlaneStages * kPlaneStageBytes + kSumScratch + kEpiStaging;
     static constexpr int kSmemBytes = kSmemData + 1024 /*align slack*/ + 1024 /*barriers*/;
-    // column sums: a thread sees kRowsPerStage rows of its 16 inputs per stage; byte lanes hold 17 rows of values <= 15,
-    // 16-bit lanes 4369 rows
-    static constexpr int kRowsPerStage = kPlaneBytes / (kUnpackThreads * 16);
-    static constexpr int kWidenStages = 16 / kRowsPerStage;
-    static constexpr int kFlushStages = 4096 / kRowsPerStage;
+    // The unpack warps work in kUnpackGroups groups; group g takes the stages it == g (mod kUnpackGroups), so several stages
+    // are unpacked at the same time and a warp's per-stage chain (barrier waits -> ld.shared -> ALU -> st.shared -> proxy
+    // fence -> arrive) is paid once per kUnpackGroups stages: with one group that chain (about 630 clk per stage) was what
+    // bounded the kernel once the diagonal tiles dropped to 2 MMAs per K-step.
+    static constexpr int kUnpackGroups = 2;
+    static constexpr int kGroupWarps = kUnpackWarps / kUnpackGroups;
+    static constexpr int kGroupThreads = kGroupWarps * 32;
+    // column sums: a thread sees kRowsPerStage rows of its 16 inputs per stage it unpacks; byte lanes hold 17 rows of values
+    // <= 15, 16-bit lanes 4369 rows
+    static constexpr int kRowsPerStage = kPlaneBytes / (kGroupThreads * 16);
+    static constexpr int kWidenStages = 16 / kRowsPerStage;                     // in stages of the thread's own group
+    static constexpr int kFlushEpoch = 1024;                                    // in stages of the segment (all groups): 2048 rows per thread
     static_assert(kUnpackThreads == 256, "the column-sum reduction assumes 256 unpack threads (32 rows x 8 chunks per pass)");
+    static_assert(kGroupThreads % 64 == 0, "a thread must keep the same 16 inputs: rows per pass must be a multiple of 8");
     static_assert(kRowsPerStage >= 1 && kRowsPerStage <= 16 && 16 % kRowsPerStage == 0, "stage size vs column-sum lanes");
+    static_assert(kFlushEpoch / kUnpackGroups * kRowsPerStage <= 4096, "16-bit column-sum lanes");
+    // mbarrier waits are by phase PARITY, which is only sound while a waiter can never be two phases ahead of the barrier.
+    // Packed ring (TMA -> unpack): the loads of different stages may land out of order, so a slot must always be consumed
+    // by the same group -- kPackedStages is a multiple of kUnpackGroups (with 3 slots and 2 groups a group could reach its
+    // next use of a slot while the other group's load into that slot was still in flight, pass the wait on the stale
+    // parity and unpack old bytes: seen as wrong visibilities on C5).  Plane ring (unpack -> MMA -> unpack): its phases
+    // complete through tcgen05.commit, in issue order, and a group has itself waited for the commit of the stage after the
+    // one in question before it comes back to a slot, so an odd ring is sound there.
+    static_assert(kPackedStages % kUnpackGroups == 0, "a packed slot must always be consumed by the same unpack group");
 };
 
 constexpr int kWarpTma = 0;
@@ -147,7 +169,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
 
     if (warp == kWarpMma && lane == 0) {
         for (int s = 0; s < Cfg::kPlaneStages; ++s) {
-            ptx::mbar_init(bar_pl_full(s), 2 * Cfg::kUnpackWarps);  // unpack warps of BOTH CTAs (used in the leader only)
+            ptx::mbar_init(bar_pl_full(s), 2 * Cfg::kGroupWarps);   // the unpack warps of one group, BOTH CTAs (used in the leader only)
             ptx::mbar_init(bar_pl_empty(s), 1);                   // tcgen05.commit (multicast to both CTAs)
         }
         ptx::mbar_init(bar_acc_full, 1);                          // tcgen05.commit (multicast)
@@ -158,7 +180,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         ptx::prefetch_tensormap(&frame_map);
         for (int s = 0; s < Cfg::kPackedStages; ++s) {
             ptx::mbar_init(bar_pk_full(s), 1);                    // TMA producer's arrive.expect_tx
-            ptx::mbar_init(bar_pk_empty(s), Cfg::kUnpackWarps);     // one arrive per unpack warp
+            ptx::mbar_init(bar_pk_empty(s), Cfg::kGroupWarps);      // one arrive per unpack warp of the stage's group
         }
         ptx::fence_mbar_init();
         ptx::fence_proxy_async_smem();
@@ -229,9 +251,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                         const uint64_t d_la = ptx::make_smem_desc_mn_sw128(pl + 1 * Cfg::kPlaneBytes + koff, 1024, 1024);
                         const uint32_t acc = (st != seg.stage_begin || k != 0) ? 1u : 0u;
                         if (!off) {
-                            ptx::mma_i8<2>(tmem_R, d_ha, d_ha, idesc, acc);   // R  = h h^T
-                            ptx::mma_i8<2>(tmem_R, d_la, d_la, idesc, 1u);    // R += l l^T
-                            ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc, acc);   // Q  = l h^T
+                            const uint64_t d_sa = ptx::make_smem_desc_mn_sw128(pl + 2 * Cfg::kPlaneBytes + koff, 1024, 1024);
+                            ptx::mma_i8<2>(tmem_R, d_sa, d_sa, idesc, acc);   // R (= G) = s s^T,  s = h + l
+                            ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc, acc);   // Q (= X) = l h^T
                         } else {
                             const uint64_t d_hb = ptx::make_smem_desc_mn_sw128(pl + 2 * Cfg::kPlaneBytes + koff, 1024, 1024);
                             const uint64_t d_lb = ptx::make_smem_desc_mn_sw128(pl + 3 * Cfg::kPlaneBytes + koff, 1024, 1024);
@@ -249,12 +271,15 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         }
     } else if (warp >= kWarpUnpack0 && warp < (uint32_t)Cfg::kWarpEpi0) {
         // ===================================================== a2: unpack warps
-        // Thread `tid` handles the 16-byte chunk at byte offset (q * 256 + tid) * 16 of every 8 KiB block: row 32 q + tid / 8,
-        // chunk position tid % 8.  TMA's 128-byte swizzle puts logical chunk c of row k at position c ^ (k % 8), so the thread
-        // always sees the same 16 inputs  [16 c_t, 16 c_t + 16),  c_t = (tid % 8) ^ ((tid / 8) % 8)  -- which is what lets it
-        // keep their column sums in registers: byte lanes (<= 16 rows), widened to 16-bit lanes (<= 4096 rows), reduced over
-        // the 32 threads that share a chunk through smem into an int32 total held by thread `input index` (< 128).
+        // A group of kGroupThreads threads unpacks a stage; thread `gtid` of the group handles the 16-byte chunks at byte offsets
+        // (q * kGroupThreads + gtid) * 16 of every 8 KiB block: row q * kGroupThreads / 8 + gtid / 8, chunk position gtid % 8.
+        // TMA's 128-byte swizzle puts logical chunk c of row k at position c ^ (k % 8), so the thread always sees the same 16
+        // inputs  [16 c_t, 16 c_t + 16),  c_t = (tid % 8) ^ ((tid / 8) % 8)  -- which is what lets it keep their column sums in
+        // registers: byte lanes (<= 16 rows), widened to 16-bit lanes (<= 4096 rows), reduced over the 32 threads that share
+        // a chunk through smem into an int32 total held by thread `input index` (< 128).
         const uint32_t tid = threadIdx.x - kWarpUnpack0 * 32;     // 0 .. 255
+        const uint32_t group = tid / Cfg::kGroupThreads;
+        const uint32_t gtid = tid % Cfg::kGroupThreads;
         const uint32_t pl_full_leader = ptx::mapa(bar_base, 0) + (bar_pl_full(0) - bar_base);
         uint32_t bsum[Cfg::kSumPlanes][4];    // byte lanes   : word k = inputs 4k .. 4k+3 of the chunk
         uint32_t wsum[Cfg::kSumPlanes][8];    // 16-bit lanes : [k] = bytes 0, 2 of word k ; [4 + k] = bytes 1, 3
@@ -310,60 +335,67 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 }
             }
         };
+        // one 8 KiB packed block -> its planes: all loads first, then unpack / sum / store row by row
+        auto load_block = [&](uint32_t src, uint32_t (&w)[Cfg::kRowsPerStage][4]) {
+#pragma unroll
+            for (int q = 0; q < Cfg::kRowsPerStage; ++q)
+                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                             : "=r"(w[q][0]), "=r"(w[q][1]), "=r"(w[q][2]), "=r"(w[q][3])
+                             : "r"(src + (uint32_t)(q * Cfg::kGroupThreads + gtid) * 16u));
+        };
+        auto st_v4 = [&](uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+        };
         uint32_t it = 0;
         for (int sg = seg_begin; sg < seg_end; ++sg) {
             const Segment seg = p.segments[sg];
             const bool off = kOffDiag && (seg.I != seg.J);
-            int since_widen = 0, since_flush = 0;
+            int since_widen = 0, epochs_done = 0;
             for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
+                if (it % Cfg::kUnpackGroups != group) continue;               // another group's stage
+                // 16-bit lanes: every thread joins a flush per kFlushEpoch stages of the segment (the same number in every group)
+                for (; epochs_done < (st - seg.stage_begin) / Cfg::kFlushEpoch; ++epochs_done) { flush(off ? 4 : 2); since_widen = 0; }
                 const uint32_t pslot = it % Cfg::kPackedStages, pph = (it / Cfg::kPackedStages) & 1u;
                 const uint32_t lslot = it % Cfg::kPlaneStages, lph = (it / Cfg::kPlaneStages) & 1u;
                 ptx::mbar_wait(bar_pk_full(pslot), pph);                      // TMA bytes landed
-                ptx::mbar_wait_cluster(bar_pl_empty(lslot), lph ^ 1u);        // MMAs that read this plane slot retired
                 const uint32_t src = smem_packed + pslot * Cfg::kPackedStageBytes;
                 const uint32_t dst = smem_planes + lslot * Cfg::kPlaneStageBytes;
+                uint32_t w[Cfg::kRowsPerStage][4];
+                load_block(src, w);
+                ptx::mbar_wait_cluster(bar_pl_empty(lslot), lph ^ 1u);        // MMAs that read this plane slot retired
 #pragma unroll
                 for (int q = 0; q < Cfg::kRowsPerStage; ++q) {
-                    const uint32_t o = (uint32_t)(q * Cfg::kUnpackThreads + tid) * 16u;
-                    uint32_t w[4], re[4], im[4];
-                    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(src + o));
+                    const uint32_t o = (uint32_t)(q * Cfg::kGroupThreads + gtid) * 16u;
+                    uint32_t re[4], im[4];
 #pragma unroll
                     for (int k = 0; k < 4; ++k) {
-                        re[k] = unpack_re4(w[k]);
-                        im[k] = unpack_im4(w[k]);
+                        re[k] = unpack_re4(w[q][k]);
+                        im[k] = unpack_im4(w[q][k]);
                         bsum[0][k] += re[k];
                         bsum[1][k] += im[k];
                     }
-                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + o), "r"(re[0]), "r"(re[1]), "r"(re[2]), "r"(re[3]) : "memory");
-                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + Cfg::kPlaneBytes + o), "r"(im[0]), "r"(im[1]), "r"(im[2]),
-                                 "r"(im[3])
-                                 : "memory");
+                    st_v4(dst + o, re[0], re[1], re[2], re[3]);
+                    st_v4(dst + Cfg::kPlaneBytes + o, im[0], im[1], im[2], im[3]);
+                    if (!off)   // diagonal super-tile: s' = h' + l' in [0, 30] per byte (no carries between bytes)
+                        st_v4(dst + 2 * Cfg::kPlaneBytes + o, re[0] + im[0], re[1] + im[1], re[2] + im[2], re[3] + im[3]);
                 }
                 if constexpr (kOffDiag) {
                     if (off) {
+                        load_block(src + Cfg::kPlaneBytes, w);
 #pragma unroll
                         for (int q = 0; q < Cfg::kRowsPerStage; ++q) {
-                            const uint32_t o = (uint32_t)(q * Cfg::kUnpackThreads + tid) * 16u;
-                            uint32_t w[4], re[4], im[4];
-                            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                                         : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3])
-                                         : "r"(src + Cfg::kPlaneBytes + o));
+                            const uint32_t o = (uint32_t)(q * Cfg::kGroupThreads + gtid) * 16u;
+                            uint32_t re[4], im[4];
 #pragma unroll
                             for (int k = 0; k < 4; ++k) {
-                                re[k] = unpack_re4(w[k]);
-                                im[k] = unpack_im4(w[k]);
+                                re[k] = unpack_re4(w[q][k]);
+                                im[k] = unpack_im4(w[q][k]);
                                 bsum[Cfg::kSumPlanes - 2][k] += re[k];
                                 bsum[Cfg::kSumPlanes - 1][k] += im[k];
                             }
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 2 * Cfg::kPlaneBytes + o), "r"(re[0]), "r"(re[1]),
-                                         "r"(re[2]), "r"(re[3])
-                                         : "memory");
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 3 * Cfg::kPlaneBytes + o), "r"(im[0]), "r"(im[1]),
-                                         "r"(im[2]), "r"(im[3])
-                                         : "memory");
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 4 * Cfg::kPlaneBytes + o), "r"(complement4(im[0])),
-                                         "r"(complement4(im[1])), "r"(complement4(im[2])), "r"(complement4(im[3]))
-                                         : "memory");
+                            st_v4(dst + 2 * Cfg::kPlaneBytes + o, re[0], re[1], re[2], re[3]);
+                            st_v4(dst + 3 * Cfg::kPlaneBytes + o, im[0], im[1], im[2], im[3]);
+                            st_v4(dst + 4 * Cfg::kPlaneBytes + o, complement4(im[0]), complement4(im[1]), complement4(im[2]), complement4(im[3]));
                         }
                     }
                 }
@@ -374,8 +406,8 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                     ptx::mbar_arrive_cluster(pl_full_leader + 8u * lslot);             // tell the leader's MMA thread
                 }
                 if (++since_widen == Cfg::kWidenStages) { widen(); since_widen = 0; }
-                if (++since_flush == Cfg::kFlushStages) { flush(off ? 4 : 2); since_flush = 0; since_widen = 0; }
             }
+            for (; epochs_done < (seg.stage_end - seg.stage_begin - 1) / Cfg::kFlushEpoch; ++epochs_done) flush(off ? 4 : 2);
             // segment done: this segment's column sums -> its sum slot (same store / load-add-store rule as the epilogue)
             ptx::grid_dependency_wait();                           // sum slots: see the note at the prologue
             flush(off ? 4 : 2);
@@ -390,8 +422,6 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                     tot[pl] = 0;
                 }
             }
-        }
-        if (tid == 0) {
         }
     } else if (warp >= (uint32_t)Cfg::kWarpEpi0) {
         // ===================================================== a4: epilogue warps

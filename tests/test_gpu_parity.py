@@ -394,6 +394,24 @@ def test_c5_full_size_stress(xb):
     assert np.array_equal(got[chans], _channels(fr, chans))
     _check_full_size(fr, got, n_samples=1200, channels=[12], n_probe=1)
     assert np.array_equal(got, run_simt(fr))             # extra
+    # steady state of long segments (2048 stages per item), many launches back to back with the promise on: the two unpack
+    # groups of a CTA drift apart and TMA loads land out of order -- a packed slot consumed by alternating groups once let a
+    # group pass its full-barrier wait on a stale phase parity here (xengine_kernel.cuh, kPackedStages % kUnpackGroups).
+    # Every launch must reproduce the result verified above.
+    x = xb.XCorr(c.n_inputs, c.n_freq, c.n_time)
+    x.promise_complete_frames()
+    dev = torch.from_numpy(fr).cuda()
+    st = torch.cuda.Stream()
+    outs = [torch.empty((c.n_freq, x.n_pairs, 2), dtype=torch.int32, device="cuda") for _ in range(12)]
+    with torch.cuda.stream(st):
+        for o in outs:
+            x.process(dev, st)
+            x.read(o, st)
+    torch.cuda.synchronize()
+    want = torch.from_numpy(got).cuda()
+    for k, o in enumerate(outs):
+        assert torch.equal(o, want), k
+    x.close()
 
 
 C3_POOL = 4   # distinct seeded 1 GiB frames, cycled 16 times = the 64 consecutive frames of BASELINE.json:configs[2]
