@@ -47,8 +47,12 @@ struct KernelCfg {
     static constexpr int kPlanes = kOffDiag ? 5 : 3;               // h_a l_a s_a   or   h_a l_a {s_a | h_b} l_b 15-l_b
     static constexpr int kPackedStageBytes = kPackedBlocks * kPlaneBytes;
     static constexpr int kPlaneStageBytes = kPlanes * kPlaneBytes;
-    static constexpr int kPackedStages = 4;
-    static constexpr int kPlaneStages = kOffDiag ? 3 : 6;
+    static constexpr int kPackedStages = kOffDiag ? 4 : 8;
+    // L2 prefetch distance of the TMA lane, in stages: the box of stage it + kPrefetchStages is requested into L2 when stage
+    // `it` is loaded into shared memory.  4 packed stages in flight per SM (4.7 MB over the chip) cover only ~2.9 TB/s at
+    // the HBM latency of this access pattern (64 rows of 128 B per box); with the prefetch the loads hit L2.
+    static constexpr int kPrefetchStages = 16;
+    static constexpr int kPlaneStages = kOffDiag ? 3 : 5;
     static constexpr int kUnpackWarps = 8;                         // multiple of 4
     static constexpr int kUnpackThreads = kUnpackWarps * 32;
     static constexpr int kWarpEpi0 = 4 + kUnpackWarps;             // epilogue warps: warp % 4 == TMEM lane quarter
@@ -63,17 +67,19 @@ struct KernelCfg {
     // are unpacked at the same time and a warp's per-stage chain (barrier waits -> ld.shared -> ALU -> st.shared -> proxy
     // fence -> arrive) is paid once per kUnpackGroups stages: with one group that chain (about 630 clk per stage) was what
     // bounded the kernel once the diagonal tiles dropped to 2 MMAs per K-step.
-    static constexpr int kUnpackGroups = 2;
+    static constexpr int kUnpackGroups = kOffDiag ? 2 : 4;
     static constexpr int kGroupWarps = kUnpackWarps / kUnpackGroups;
     static constexpr int kGroupThreads = kGroupWarps * 32;
     // column sums: a thread sees kRowsPerStage rows of its 16 inputs per stage it unpacks; byte lanes hold 17 rows of values
     // <= 15, 16-bit lanes 4369 rows
     static constexpr int kRowsPerStage = kPlaneBytes / (kGroupThreads * 16);
+    static constexpr int kLoadBatch = 4;                                        // rows (16-byte loads) a thread has in flight at a time
     static constexpr int kWidenStages = 16 / kRowsPerStage;                     // in stages of the thread's own group
     static constexpr int kFlushEpoch = 1024;                                    // in stages of the segment (all groups): 2048 rows per thread
     static_assert(kUnpackThreads == 256, "the column-sum reduction assumes 256 unpack threads (32 rows x 8 chunks per pass)");
     static_assert(kGroupThreads % 64 == 0, "a thread must keep the same 16 inputs: rows per pass must be a multiple of 8");
     static_assert(kRowsPerStage >= 1 && kRowsPerStage <= 16 && 16 % kRowsPerStage == 0, "stage size vs column-sum lanes");
+    static_assert(kRowsPerStage % kLoadBatch == 0, "rows per stage vs load batch");
     static_assert(kFlushEpoch / kUnpackGroups * kRowsPerStage <= 4096, "16-bit column-sum lanes");
     // mbarrier waits are by phase PARITY, which is only sound while a waiter can never be two phases ahead of the barrier.
     // Packed ring (TMA -> unpack): the loads of different stages may land out of order, so a slot must always be consumed
@@ -165,6 +171,21 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         if (off)
             ptx::tma_load_3d(dst + Cfg::kPlaneBytes, &frame_map, bar_pk_full(slot), seg.J * kSuper + (int)rank * kBlock, seg.f, st * kStageT);
     };
+    // the same box requested into L2 only
+    auto tma_prefetch = [&](const Segment &seg, int st) {
+        ptx::tma_prefetch_3d(&frame_map, seg.I * kSuper + (int)rank * kBlock, seg.f, st * kStageT);
+        if (kOffDiag && (seg.I != seg.J)) ptx::tma_prefetch_3d(&frame_map, seg.J * kSuper + (int)rank * kBlock, seg.f, st * kStageT);
+    };
+    // cursor of the L2 prefetch: runs kPrefetchStages stages ahead of the loads through the worker's segment list
+    int pf_sg = seg_begin, pf_st = 0;
+    Segment pf_seg = {};
+    auto prefetch_next = [&]() {
+        if (pf_sg >= seg_end) return;
+        tma_prefetch(pf_seg, pf_st);
+        if (++pf_st >= pf_seg.stage_end) {
+            if (++pf_sg < seg_end) { pf_seg = p.segments[pf_sg]; pf_st = pf_seg.stage_begin; }
+        }
+    };
     uint32_t tma_pre = 0;   // packed stages the TMA lane put in flight before the prologue barrier (their slots start empty)
 
     if (warp == kWarpMma && lane == 0) {
@@ -189,6 +210,8 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         // the frame may be the output of the previous kernel of the stream, which may have let this grid start early:
         // wait for it, unless the caller has promised complete frames (xcorr_promise_complete_frames)
         if (p.wait_frame) ptx::grid_dependency_wait();
+        if (pf_sg < seg_end) { pf_seg = p.segments[pf_sg]; pf_st = pf_seg.stage_begin; }
+        for (int k = 0; k < Cfg::kPrefetchStages; ++k) prefetch_next();
         for (int sg = seg_begin; sg < seg_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++sg) {
             const Segment seg = p.segments[sg];
             for (int st = seg.stage_begin; st < seg.stage_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++st, ++tma_pre)
@@ -218,6 +241,7 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             for (int sg = seg_begin; sg < seg_end; ++sg) {
                 const Segment seg = p.segments[sg];
                 for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
+                    prefetch_next();                               // stage it + kPrefetchStages -> L2
                     if (it < tma_pre) continue;                    // already in flight (prologue)
                     const uint32_t slot = it % Cfg::kPackedStages;
                     const uint32_t ph = (it / Cfg::kPackedStages) & 1u;
@@ -335,13 +359,13 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 }
             }
         };
-        // one 8 KiB packed block -> its planes: all loads first, then unpack / sum / store row by row
-        auto load_block = [&](uint32_t src, uint32_t (&w)[Cfg::kRowsPerStage][4]) {
+        // one 8 KiB packed block -> its planes, kLoadBatch rows at a time: the batch's loads first, then unpack / sum / store
+        auto load_batch = [&](uint32_t src, int q0, uint32_t (&w)[Cfg::kLoadBatch][4]) {
 #pragma unroll
-            for (int q = 0; q < Cfg::kRowsPerStage; ++q)
+            for (int q = 0; q < Cfg::kLoadBatch; ++q)
                 asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
                              : "=r"(w[q][0]), "=r"(w[q][1]), "=r"(w[q][2]), "=r"(w[q][3])
-                             : "r"(src + (uint32_t)(q * Cfg::kGroupThreads + gtid) * 16u));
+                             : "r"(src + (uint32_t)((q0 + q) * Cfg::kGroupThreads + gtid) * 16u));
         };
         auto st_v4 = [&](uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
             asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
@@ -360,42 +384,49 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 ptx::mbar_wait(bar_pk_full(pslot), pph);                      // TMA bytes landed
                 const uint32_t src = smem_packed + pslot * Cfg::kPackedStageBytes;
                 const uint32_t dst = smem_planes + lslot * Cfg::kPlaneStageBytes;
-                uint32_t w[Cfg::kRowsPerStage][4];
-                load_block(src, w);
+                uint32_t w[Cfg::kLoadBatch][4];
+                load_batch(src, 0, w);
                 ptx::mbar_wait_cluster(bar_pl_empty(lslot), lph ^ 1u);        // MMAs that read this plane slot retired
 #pragma unroll
-                for (int q = 0; q < Cfg::kRowsPerStage; ++q) {
-                    const uint32_t o = (uint32_t)(q * Cfg::kGroupThreads + gtid) * 16u;
-                    uint32_t re[4], im[4];
+                for (int q0 = 0; q0 < Cfg::kRowsPerStage; q0 += Cfg::kLoadBatch) {
+                    if (q0 > 0) load_batch(src, q0, w);
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        re[k] = unpack_re4(w[q][k]);
-                        im[k] = unpack_im4(w[q][k]);
-                        bsum[0][k] += re[k];
-                        bsum[1][k] += im[k];
+                    for (int q = 0; q < Cfg::kLoadBatch; ++q) {
+                        const uint32_t o = (uint32_t)((q0 + q) * Cfg::kGroupThreads + gtid) * 16u;
+                        uint32_t re[4], im[4];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            re[k] = unpack_re4(w[q][k]);
+                            im[k] = unpack_im4(w[q][k]);
+                            bsum[0][k] += re[k];
+                            bsum[1][k] += im[k];
+                        }
+                        st_v4(dst + o, re[0], re[1], re[2], re[3]);
+                        st_v4(dst + Cfg::kPlaneBytes + o, im[0], im[1], im[2], im[3]);
+                        if (!off)   // diagonal super-tile: s' = h' + l' in [0, 30] per byte (no carries between bytes)
+                            st_v4(dst + 2 * Cfg::kPlaneBytes + o, re[0] + im[0], re[1] + im[1], re[2] + im[2], re[3] + im[3]);
                     }
-                    st_v4(dst + o, re[0], re[1], re[2], re[3]);
-                    st_v4(dst + Cfg::kPlaneBytes + o, im[0], im[1], im[2], im[3]);
-                    if (!off)   // diagonal super-tile: s' = h' + l' in [0, 30] per byte (no carries between bytes)
-                        st_v4(dst + 2 * Cfg::kPlaneBytes + o, re[0] + im[0], re[1] + im[1], re[2] + im[2], re[3] + im[3]);
                 }
                 if constexpr (kOffDiag) {
                     if (off) {
-                        load_block(src + Cfg::kPlaneBytes, w);
 #pragma unroll
-                        for (int q = 0; q < Cfg::kRowsPerStage; ++q) {
-                            const uint32_t o = (uint32_t)(q * Cfg::kGroupThreads + gtid) * 16u;
-                            uint32_t re[4], im[4];
+                        for (int q0 = 0; q0 < Cfg::kRowsPerStage; q0 += Cfg::kLoadBatch) {
+                            load_batch(src + Cfg::kPlaneBytes, q0, w);
 #pragma unroll
-                            for (int k = 0; k < 4; ++k) {
-                                re[k] = unpack_re4(w[q][k]);
-                                im[k] = unpack_im4(w[q][k]);
-                                bsum[Cfg::kSumPlanes - 2][k] += re[k];
-                                bsum[Cfg::kSumPlanes - 1][k] += im[k];
+                            for (int q = 0; q < Cfg::kLoadBatch; ++q) {
+                                const uint32_t o = (uint32_t)((q0 + q) * Cfg::kGroupThreads + gtid) * 16u;
+                                uint32_t re[4], im[4];
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) {
+                                    re[k] = unpack_re4(w[q][k]);
+                                    im[k] = unpack_im4(w[q][k]);
+                                    bsum[Cfg::kSumPlanes - 2][k] += re[k];
+                                    bsum[Cfg::kSumPlanes - 1][k] += im[k];
+                                }
+                                st_v4(dst + 2 * Cfg::kPlaneBytes + o, re[0], re[1], re[2], re[3]);
+                                st_v4(dst + 3 * Cfg::kPlaneBytes + o, im[0], im[1], im[2], im[3]);
+                                st_v4(dst + 4 * Cfg::kPlaneBytes + o, complement4(im[0]), complement4(im[1]), complement4(im[2]), complement4(im[3]));
                             }
-                            st_v4(dst + 2 * Cfg::kPlaneBytes + o, re[0], re[1], re[2], re[3]);
-                            st_v4(dst + 3 * Cfg::kPlaneBytes + o, im[0], im[1], im[2], im[3]);
-                            st_v4(dst + 4 * Cfg::kPlaneBytes + o, complement4(im[0]), complement4(im[1]), complement4(im[2]), complement4(im[3]));
                         }
                     }
                 }
