@@ -89,6 +89,20 @@ size_t xcorr_assembler_packet_bytes(const xcorr_assembler *a);
 int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_packets, uint64_t seq0, void *frame_dev,
                    uint8_t *flags_dev, int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream);
 
+/*
+ * xcorr_assemble_accounted -- xcorr_assemble() and xcorr_norm_process_dev() in ONE pass over the packets: the F-engine
+ * flags of the footers ("the bit-field ... is read initially as 32-bit integers, and bit-field extraction is performed
+ * only if ... non-zero") are counted into the handle's flag / intersection accumulator while they pass
+ * through assemble_kernel's registers, and the packet-loss counters (:113, :115) go straight into the handle's.  The flag
+ * field need not exist in memory at all: `flags_dev` and `lost_dev` are optional outputs here (NULL to skip).
+ *
+ *   h   a handle of the same N, F, T on the same device with xcorr_norm_enable() done; its accumulators are added to on
+ *       `cuda_stream` (stream order with the handle's other calls as described in xcorr.h).
+ * Everything else as in xcorr_assemble().  Errors: EINVAL (also: normalisation not enabled, shapes differ), ECUDA.
+ */
+int xcorr_assemble_accounted(xcorr_assembler *a, xcorr_handle *h, const void *packets, size_t n_packets, uint64_t seq0,
+                             void *frame_dev, uint8_t *flags_dev, int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream);
+
 /* Total number of this library's kernels launched through the assembler so far. */
 uint64_t xcorr_assembler_kernel_launches(const xcorr_assembler *a);
 
@@ -114,7 +128,7 @@ int xcorr_norm_process_dev(xcorr_handle *h, const uint8_t *flags_dev, const int3
 
 /*
  * xcorr_stream_attach_assembler -- startup-time call: gives the stream's `depth` ring slots a device buffer for
- * `max_packets` packets, a flag field and loss counters.  `a` (same N, F, T as the stream's handle) is BORROWED
+ * `max_packets` packets.  `a` (same N, F, T as the stream's handle) is BORROWED
  * until the stream is destroyed.  Once per stream.  Errors: EINVAL, ENOMEM.
  */
 int xcorr_stream_attach_assembler(xcorr_stream *s, xcorr_assembler *a, size_t max_packets);
@@ -122,8 +136,8 @@ int xcorr_stream_attach_assembler(xcorr_stream *s, xcorr_assembler *a, size_t ma
 /*
  * xcorr_stream_submit_packets -- enqueue one frame given as its packets in arrival order (page-locked host memory,
  * n_packets <= max_packets, layout as for xcorr_assemble): H2D copy on the copy stream, then on the compute stream
- * xcorr_assemble -> xcorr_process and, if the handle has normalisation enabled, xcorr_norm_process_dev with the
- * frame's flag field and loss counters.  `packets_host` is BORROWED until the copy has completed (as in
+ * xcorr_assemble -> xcorr_process; if the handle has normalisation enabled the assembly is xcorr_assemble_accounted, i.e.
+ * the frame's flags and packet losses are accounted in the same pass.  `packets_host` is BORROWED until the copy has completed (as in
  * xcorr_stream_submit).  Returns without waiting unless all ring slots are in flight.
  * Errors: EINVAL, EOVERFLOW, ECUDA.
  */

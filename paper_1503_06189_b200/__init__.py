@@ -19,7 +19,7 @@ __all__ = [
     "xcorr_norm_enable", "xcorr_norm_process", "xcorr_read_normalized", "xcorr_promise_complete_frames",
     "xcorr_stream_create", "xcorr_stream_submit", "xcorr_stream_sync", "xcorr_stream_read", "xcorr_stream_read_async", "xcorr_stream_destroy",
     "xcorr_assembler_create", "xcorr_assembler_packet_bytes", "xcorr_assemble", "xcorr_assembler_kernel_launches",
-    "xcorr_assembler_destroy", "xcorr_norm_process_dev", "xcorr_stream_attach_assembler", "xcorr_stream_submit_packets",
+    "xcorr_assembler_destroy", "xcorr_norm_process_dev", "xcorr_assemble_accounted", "xcorr_stream_attach_assembler", "xcorr_stream_submit_packets",
     "xcorr_stream_read_normalized",
     "xcorr_debug_schedule", "xcorr_debug_stage_samples", "XCorr", "XCorrStream", "Assembler",
 ]
@@ -97,6 +97,8 @@ def lib() -> ctypes.CDLL:
     L.xcorr_assembler_packet_bytes.restype = ctypes.c_size_t
     L.xcorr_assemble.argtypes = [vp, vp, ctypes.c_size_t, ctypes.c_uint64, vp, vp, vp, vp, vp]
     L.xcorr_assemble.restype = ci
+    L.xcorr_assemble_accounted.argtypes = [vp, vp, vp, ctypes.c_size_t, ctypes.c_uint64, vp, vp, vp, vp, vp]
+    L.xcorr_assemble_accounted.restype = ci
     L.xcorr_assembler_kernel_launches.argtypes = [vp]
     L.xcorr_assembler_kernel_launches.restype = ctypes.c_uint64
     L.xcorr_assembler_destroy.argtypes = [vp]
@@ -193,6 +195,12 @@ def xcorr_assemble(assembler: int, packets: int, n_packets: int, seq0: int, fram
                    counts_dev: int = 0, cuda_stream: int = 0) -> int:
     return lib().xcorr_assemble(assembler, packets or None, int(n_packets), int(seq0), frame_dev or None, flags_dev or None,
                                 lost_dev or None, counts_dev or None, cuda_stream)
+
+
+def xcorr_assemble_accounted(assembler: int, handle: int, packets: int, n_packets: int, seq0: int, frame_dev: int, flags_dev: int = 0,
+                             lost_dev: int = 0, counts_dev: int = 0, cuda_stream: int = 0) -> int:
+    return lib().xcorr_assemble_accounted(assembler, handle, packets or None, int(n_packets), int(seq0), frame_dev or None,
+                                          flags_dev or None, lost_dev or None, counts_dev or None, cuda_stream)
 
 
 def xcorr_assembler_kernel_launches(assembler: int) -> int:
@@ -455,9 +463,11 @@ class Assembler:
     def kernel_launches(self) -> int:
         return xcorr_assembler_kernel_launches(self.handle)
 
-    def assemble(self, packets, n_packets: int, seq0: int, frame=None, flags=None, lost=None, counts=None, stream=None):
+    def assemble(self, packets, n_packets: int, seq0: int, frame=None, flags=None, lost=None, counts=None, stream=None, account_into=None):
         """packets: CUDA or pinned-CPU uint8 tensor holding >= n_packets packets back to back (arrival order).
-        frame / flags / lost / counts: CUDA output tensors (allocated if None).  -> (frame, flags, lost, counts)."""
+        frame / flags / lost / counts: CUDA output tensors (allocated if None).  -> (frame, flags, lost, counts).
+        account_into: an ``XCorr`` with normalisation enabled -> xcorr_assemble_accounted (flags and losses are counted into
+        that handle in the same pass; no separate norm_process call is needed)."""
         import torch
         if packets is not None and packets.numel() * packets.element_size() < n_packets * self.packet_bytes:
             raise ValueError("packets holds fewer than n_packets packets")
@@ -470,8 +480,13 @@ class Assembler:
         counts = torch.empty(4, dtype=torch.int32, device="cuda") if counts is None else counts
         if frame.numel() != t * f * n or flags.numel() * 8 != t * f * n or lost.numel() != f or counts.numel() != 4:
             raise ValueError("output tensor of the wrong size")
-        rc = xcorr_assemble(self.handle, packets.data_ptr() if packets is not None else 0, n_packets, seq0, frame.data_ptr(),
-                            flags.data_ptr(), lost.data_ptr(), counts.data_ptr(), _stream_handle(stream))
+        pptr = packets.data_ptr() if packets is not None else 0
+        if account_into is None:
+            rc = xcorr_assemble(self.handle, pptr, n_packets, seq0, frame.data_ptr(), flags.data_ptr(), lost.data_ptr(), counts.data_ptr(),
+                                _stream_handle(stream))
+        else:
+            rc = xcorr_assemble_accounted(self.handle, account_into.handle, pptr, n_packets, seq0, frame.data_ptr(), flags.data_ptr(),
+                                          lost.data_ptr(), counts.data_ptr(), _stream_handle(stream))
         if rc != XCORR_OK:
             raise XCorrError(rc, "xcorr_assemble")
         return frame, flags, lost, counts

@@ -16,10 +16,18 @@
 //                         the channels' packet-loss counters (:113, P6).  Every byte of the frame and of the flag field
 //                         is written exactly once: no clearing pass.
 //
-// HBM-bound: per frame, reads n_packets * packet_bytes, writes T*F*N + T*F*N/8.
+//                         With kAccount (xcorr_assemble_accounted) the same pass also does the flag / loss accounting of
+//                         the lost-sample normalisation (normalise_kernel.cuh; PAPER.md:113-:123): every footer word is in
+//                         a register here anyway, so a non-zero one is expanded on the spot into the handle's intersection /
+//                         counter accumulator X, and the loss counters go straight into the handle's -- the flag field need
+//                         not be written to memory and read back by flag_count_kernel at all.
+//
+// HBM-bound: per frame, reads n_packets * packet_bytes, writes T*F*N (+ T*F*N/8 if the flag field is wanted).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
+
+#include "layout.hpp"
 
 namespace xc {
 
@@ -66,11 +74,47 @@ __global__ void __launch_bounds__(256) packet_claim_kernel(const uint8_t *__rest
 // 4 flag bits -> 4 byte masks (0xFF where flagged): bit k of x goes to bit 8k (the partial products never collide)
 __device__ __forceinline__ uint32_t spread4(uint32_t x) { return (((x & 0xFu) * 0x00204081u) & 0x01010101u) * 0xFFu; }
 
+// kAccount: the flag bits of one 16-byte footer chunk (row `dt` of the position, chunk `w` of that row's C * N / 8 bytes) ->
+// X[f][p(n, j)] += 1 for every flagged input n of the chunk and every input j >= n flagged in the same sample (j == n is the
+// flag counter c_f[n] on the diagonal): the paper's O(E^2) intersection tracking (:117-:119, :123), done by the thread that
+// holds the chunk.  `row_bits` = the footer bytes of row dt (C samples of N / 8 bytes each, in the packet).
+__device__ __forceinline__ void account_flag_chunk(const uint4 v, const uint8_t *__restrict__ row_bits, unsigned w, int n_inputs, int f_base,
+                                                   int32_t *__restrict__ x)
+{
+    const long long n_pairs = (long long)n_inputs * (n_inputs + 1) / 2;
+    const int n_half = n_inputs >> 4;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        uint32_t m = (q == 0) ? v.x : (q == 1) ? v.y : (q == 2) ? v.z : v.w;
+        while (m) {
+            const int b = __ffs((int)m) - 1;
+            m &= m - 1;
+            const unsigned idx = w * 128u + 32u * (unsigned)q + (unsigned)b;      // bit index inside the row
+            const int ch = (int)(idx / (unsigned)n_inputs), n = (int)(idx % (unsigned)n_inputs);
+            const uint16_t *sample = reinterpret_cast<const uint16_t *>(row_bits + (size_t)ch * (size_t)(n_inputs >> 3));
+            int32_t *x_f = x + (size_t)(f_base + ch) * (size_t)n_pairs;
+            const long long row = pair_index(n_inputs, n, n) - n;                 // p(n, j) = row + j
+            for (int k = n >> 4; k < n_half; ++k) {
+                uint32_t bits = __ldg(sample + k);
+                if (k == (n >> 4)) bits &= 0xFFFFu << (n & 15);                   // only j >= n
+                while (bits) {
+                    const int b2 = __ffs((int)bits) - 1;
+                    bits &= bits - 1;
+                    atomicAdd(x_f + row + (16 * k + b2), 1);
+                }
+            }
+        }
+    }
+}
+
+// kAccount = false: xcorr_assemble.  kAccount = true: xcorr_assemble_accounted -- `x` = the handle's intersection / counter
+// accumulator int32[F][P], `lost_acc` = its per-channel loss counters (both added to).
+template <bool kAccount>
 __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict__ packets, AssembleShape sh,
                                                         const uint32_t *__restrict__ owner, uint32_t *__restrict__ owner_next,
                                                         uint8_t *__restrict__ frame,
                                                         uint8_t *__restrict__ flags, int32_t *__restrict__ lost, uint32_t *__restrict__ counts,
-                                                        uint32_t *__restrict__ counts_out)
+                                                        uint32_t *__restrict__ counts_out, int32_t *__restrict__ x, int32_t *__restrict__ lost_acc)
 {
     const int N = sh.n_inputs, F = sh.n_freq, S = sh.s_per_packet, C = sh.c_per_packet;
     const unsigned row_chunks = (unsigned)(C * N) >> 4;            // 16-byte vectors per time sample of one stream
@@ -116,12 +160,19 @@ __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict
                     frame_v[dt1 * frame_row_stride + w1] = v1;
                 }
             }
-            if (flags) {
+            if (flags || kAccount) {
                 const uint4 *foot = reinterpret_cast<const uint4 *>(foot16);
                 uint4 *flags_v = reinterpret_cast<uint4 *>(flags + (f0 >> 3));
                 for (unsigned c = threadIdx.x; c < foot_chunks; c += blockDim.x) {
                     const unsigned dt = c / frow_chunks, w = c - dt * frow_chunks;
-                    flags_v[dt * (frame_row_stride >> 3) + w] = __ldg(foot + c);
+                    const uint4 v = __ldg(foot + c);
+                    if (flags) flags_v[dt * (frame_row_stride >> 3) + w] = v;
+                    if constexpr (kAccount) {
+                        // "read initially as 32-bit integers, and bit-field extraction is performed only if ... non-zero" (:123)
+                        if (v.x | v.y | v.z | v.w)
+                            account_flag_chunk(v, reinterpret_cast<const uint8_t *>(foot) + (size_t)dt * ((size_t)(C * N) >> 3), w, N,
+                                               C * (int)stream, x);
+                    }
                 }
             }
             kept_local += 1;
@@ -140,6 +191,9 @@ __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict
                 }
             }
             if (lost && threadIdx.x < (unsigned)C) atomicAdd(lost + C * stream + threadIdx.x, S);   // packet-loss counter (P6)
+            if constexpr (kAccount) {
+                if (threadIdx.x < (unsigned)C) atomicAdd(lost_acc + C * stream + threadIdx.x, S);
+            }
             lost_local += 1;
         }
     }

@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
                 // L = lost + c_i + c_j - X_ij (the point (i, i) receives its counter once); V~ = V * T / (T - L)
                 const int32_t x_ii = sC[0][ic];
                 int32_t x_ij = 0;
-                if (i != j) {
+                if (i != j && x_ii != 0 && x_jj != 0) {   // two inputs are flagged together at most as often as either one is: X_ij <= min(c_i, c_j)
                     x_ij = np.x[p];
                     if (x_ij) np.x[p] = 0;             // ends the integration: this thread is the only reader of X[p]
                 }

@@ -82,8 +82,6 @@ struct xcorr_stream {
     struct xcorr_assembler *assembler = nullptr;   // borrowed
     size_t max_packets = 0;
     uint8_t *pkt_buf[8] = {};
-    uint8_t *flags_buf[8] = {};
-    int32_t *lost_buf[8] = {};
 };
 
 #define XC_CUDA(h, expr)                                  \
@@ -547,8 +545,6 @@ extern "C" void xcorr_stream_destroy(xcorr_stream *s)
     for (int k = 0; k < s->depth; ++k) {
         if (s->buf[k]) cudaFree(s->buf[k]);
         if (s->pkt_buf[k]) cudaFree(s->pkt_buf[k]);
-        if (s->flags_buf[k]) cudaFree(s->flags_buf[k]);
-        if (s->lost_buf[k]) cudaFree(s->lost_buf[k]);
         if (s->copied[k]) cudaEventDestroy(s->copied[k]);
         if (s->consumed[k]) cudaEventDestroy(s->consumed[k]);
     }
@@ -715,8 +711,8 @@ extern "C" int xcorr_assembler_create(int n_inputs, int n_freq, int t_per_frame,
     return XCORR_OK;
 }
 
-extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_packets, uint64_t seq0, void *frame_dev,
-                              uint8_t *flags_dev, int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream)
+static int assemble_common(xcorr_assembler *a, xcorr_handle *h, const void *packets, size_t n_packets, uint64_t seq0, void *frame_dev,
+                           uint8_t *flags_dev, int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream)
 {
     if (!a || !frame_dev || (!packets && n_packets) || n_packets > 0x7FFFFFFEull) return XCORR_EINVAL;
     if (((uintptr_t)packets & 15u) || ((uintptr_t)frame_dev & 15u) || ((uintptr_t)flags_dev & 15u) || ((uintptr_t)lost_dev & 3u) ||
@@ -725,6 +721,12 @@ extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_
     cudaStream_t s = (cudaStream_t)cuda_stream;
     {
         const int rc = check_device(a->device);
+        if (rc != XCORR_OK) return rc;
+    }
+    if (h) {   // accounted form: the handle's flag / loss accumulators are written by assemble_kernel on this stream
+        if (!h->norm || h->device != a->device || h->n_inputs != a->sh.n_inputs || h->n_freq != a->sh.n_freq || h->n_time != a->sh.n_time)
+            return XCORR_EINVAL;
+        const int rc = order_after_previous(h, s);
         if (rc != XCORR_OK) return rc;
     }
     // no memsets: the ownership tables and counters are left clean by the previous call's assemble_kernel (see create)
@@ -740,12 +742,33 @@ extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_
     // grid-stride over the positions: 8 resident CTAs of 256 threads per SM
     unsigned blocks = (unsigned)a->n_sms * 8u;
     if (blocks > a->n_positions) blocks = a->n_positions;
-    assemble_kernel<<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, owner, owner_next, (uint8_t *)frame_dev, flags_dev, lost_dev,
-                                           a->counts, counts_dev);
+    if (h)
+        assemble_kernel<true><<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, owner, owner_next, (uint8_t *)frame_dev, flags_dev,
+                                                     lost_dev, a->counts, counts_dev, h->flag_x, h->lost_dev_acc);
+    else
+        assemble_kernel<false><<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, owner, owner_next, (uint8_t *)frame_dev, flags_dev,
+                                                      lost_dev, a->counts, counts_dev, nullptr, nullptr);
     XC_CUDA(a, cudaGetLastError());
     a->launches += 1;
     a->calls += 1;   // the tables swap roles only once both kernels are in the stream
+    if (h) {
+        h->flags_dirty = true;
+        h->lost_dev_dirty = true;
+    }
     return XCORR_OK;
+}
+
+extern "C" int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_packets, uint64_t seq0, void *frame_dev,
+                              uint8_t *flags_dev, int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream)
+{
+    return assemble_common(a, nullptr, packets, n_packets, seq0, frame_dev, flags_dev, lost_dev, counts_dev, cuda_stream);
+}
+
+extern "C" int xcorr_assemble_accounted(xcorr_assembler *a, xcorr_handle *h, const void *packets, size_t n_packets, uint64_t seq0,
+                                        void *frame_dev, uint8_t *flags_dev, int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream)
+{
+    if (!h) return XCORR_EINVAL;
+    return assemble_common(a, h, packets, n_packets, seq0, frame_dev, flags_dev, lost_dev, counts_dev, cuda_stream);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -757,9 +780,7 @@ extern "C" int xcorr_stream_attach_assembler(xcorr_stream *s, xcorr_assembler *a
     xcorr_handle *h = s->h;
     if (a->sh.n_inputs != h->n_inputs || a->sh.n_freq != h->n_freq || a->sh.n_time != h->n_time) return XCORR_EINVAL;
     for (int k = 0; k < s->depth; ++k) {
-        if (cudaMalloc(&s->pkt_buf[k], max_packets * (size_t)a->sh.packet_bytes) != cudaSuccess ||
-            cudaMalloc(&s->flags_buf[k], h->frame_bytes / 8) != cudaSuccess ||
-            cudaMalloc(&s->lost_buf[k], sizeof(int32_t) * h->n_freq) != cudaSuccess) {
+        if (cudaMalloc(&s->pkt_buf[k], max_packets * (size_t)a->sh.packet_bytes) != cudaSuccess) {
             h->last_cuda_error = (int)cudaGetLastError();
             return XCORR_ENOMEM;
         }
@@ -782,14 +803,12 @@ extern "C" int xcorr_stream_submit_packets(xcorr_stream *s, const void *packets_
                                    s->copy_stream));
     XC_CUDA(h, cudaEventRecord(s->copied[k], s->copy_stream));
     XC_CUDA(h, cudaStreamWaitEvent(s->compute_stream, s->copied[k], 0));
-    int rc = xcorr_assemble(a, s->pkt_buf[k], n_packets, seq0, s->buf[k], s->flags_buf[k], s->lost_buf[k], nullptr, (void *)s->compute_stream);
+    // with normalisation enabled the flag / loss accounting happens inside assemble_kernel (no flag field is materialised)
+    int rc = assemble_common(a, h->norm ? h : nullptr, s->pkt_buf[k], n_packets, seq0, s->buf[k], nullptr, nullptr, nullptr,
+                             (void *)s->compute_stream);
     if (rc != XCORR_OK) return rc;
     rc = xcorr_process(h, s->buf[k], (void *)s->compute_stream);
     if (rc != XCORR_OK) return rc;
-    if (h->norm) {
-        rc = xcorr_norm_process_dev(h, s->flags_buf[k], s->lost_buf[k], (void *)s->compute_stream);
-        if (rc != XCORR_OK) return rc;
-    }
     XC_CUDA(h, cudaEventRecord(s->consumed[k], s->compute_stream));
     s->submitted += 1;
     return XCORR_OK;

@@ -76,6 +76,7 @@ def test_assembler_null_handles_are_harmless():
     assert xb.xcorr_assembler_kernel_launches(0) == 0
     xb.xcorr_assembler_destroy(0)
     assert xb.xcorr_assemble(0, 0, 0, 0, 0) == xb.XCORR_EINVAL
+    assert xb.xcorr_assemble_accounted(0, 0, 0, 0, 0, 0) == xb.XCORR_EINVAL
     assert xb.xcorr_norm_process_dev(0, 0, 0, 0) == xb.XCORR_EINVAL
     assert xb.xcorr_stream_attach_assembler(0, 0, 16) == xb.XCORR_EINVAL
     assert xb.xcorr_stream_submit_packets(0, 0, 0, 0) == xb.XCORR_EINVAL

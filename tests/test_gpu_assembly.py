@@ -157,6 +157,46 @@ def test_assemble_then_process_with_promise_on_one_stream(xb):
     a.close(); x.close()
 
 
+def test_assemble_accounted_equals_assemble_plus_norm_process(xb):
+    """xcorr_assemble_accounted: flags and packet losses counted inside assemble_kernel.  Same L (bit-exact) and the same
+    normalised visibilities as the oracles chained; the optional flag field / loss counters it can still write are exact too.
+    Dense flags (bursts with many inputs flagged together) so that the O(E^2) intersection path runs, two frames, N with
+    several 16-byte footer chunks per sample (272) and with several samples per chunk (16, 48)."""
+    for (n, f, t) in [(272, 16, 64), (48, 16, 128), (16, 8, 64)]:
+        x = xb.XCorr(n, f, t)
+        x.norm_enable()
+        a = xb.Assembler(n, f, t)
+        vis = np.zeros((f, n * (n + 1) // 2, 2), dtype=np.int64)
+        flags_all, lost_all = [], np.zeros(f, dtype=np.int64)
+        for k in range(2):
+            fr = wl.make_frame("gaussian", n, f, t, 400 + k)
+            fl, _, _ = wl.draw_flags_and_loss(n, f, t, 410 + k, p_flag=0.02, p_burst=0.05, burst_frac=0.3, p_packet_loss=0.0)
+            pk = wl.packetise(fr, wl.pack_flags(fl), 7_000 + k * t)
+            arrived = wl.disturb_packets(pk, 420 + k, p_loss=0.1, p_dup=0.05, p_late=0.1, n_foreign=4)
+            want = oa.assemble(arrived, n, f, t, 7_000 + k * t)
+            frame, flags, lost, counts = a.assemble(torch.from_numpy(arrived.reshape(-1)).cuda(), arrived.shape[0], 7_000 + k * t,
+                                                    account_into=x)
+            x.process(frame)
+            check((frame.cpu().numpy(), flags.cpu().numpy(), lost.cpu().numpy(), counts.cpu().numpy()), want)
+            vis += oracle.planar(want["frame"]).astype(np.int64)
+            flags_all.append(np.unpackbits(want["flags"], axis=-1, bitorder="little").astype(bool))
+            lost_all += want["lost"]
+        L = torch.empty((f, n * (n + 1) // 2), dtype=torch.int32, device="cuda")
+        got = x.read_normalized(lost_out=L).cpu().numpy()
+        want_L = on.lost_matrix(np.concatenate(flags_all, axis=0), lost_all)
+        assert np.array_equal(L.cpu().numpy().astype(np.int64), want_L)
+        want_v = on.normalise(vis, 2 * t, want_L)
+        assert np.all(np.abs(got - want_v) <= 2.0 ** -22 * np.abs(want_v))
+        # the read ended the integration for the accumulators the assembler writes into as well
+        frame, _, _, _ = a.assemble(None, 0, 0, account_into=x)
+        x.process(frame)
+        x.read_normalized(lost_out=L)
+        assert (L.cpu().numpy() == t).all()                 # nothing arrived: every sample of every channel lost, no flags
+        with pytest.raises(xb.XCorrError):
+            a.assemble(None, 0, 0, account_into=xb.XCorr(n, f, t))     # normalisation not enabled on that handle
+        a.close(); x.close()
+
+
 @pytest.mark.parametrize("promise", [False, True])
 def test_streamed_packet_path(xb, promise):
     """Pinned packet rings -> xcorr_stream_submit_packets (H2D, assemble, correlate, flag / loss accounting) x 5 frames over a
