@@ -28,6 +28,7 @@
 #include <cuda_runtime.h>
 
 #include "layout.hpp"
+#include "normalise_kernel.cuh"
 
 namespace xc {
 
@@ -74,34 +75,33 @@ __global__ void __launch_bounds__(256) packet_claim_kernel(const uint8_t *__rest
 // 4 flag bits -> 4 byte masks (0xFF where flagged): bit k of x goes to bit 8k (the partial products never collide)
 __device__ __forceinline__ uint32_t spread4(uint32_t x) { return (((x & 0xFu) * 0x00204081u) & 0x01010101u) * 0xFFu; }
 
-// kAccount: the flag bits of one 16-byte footer chunk (row `dt` of the position, chunk `w` of that row's C * N / 8 bytes) ->
-// X[f][p(n, j)] += 1 for every flagged input n of the chunk and every input j >= n flagged in the same sample (j == n is the
-// flag counter c_f[n] on the diagonal): the paper's O(E^2) intersection tracking (:117-:119, :123), done by the thread that
-// holds the chunk.  `row_bits` = the footer bytes of row dt (C samples of N / 8 bytes each, in the packet).
-__device__ __forceinline__ void account_flag_chunk(const uint4 v, const uint8_t *__restrict__ row_bits, unsigned w, int n_inputs, int f_base,
-                                                   int32_t *__restrict__ x)
+// kAccount, the rare path: some lanes of the warp hold footer chunks (16 bytes = 128 flag bits each, chunk cw + lane of the
+// position) with flags set (mask nz).  "read initially as 32-bit integers, and bit-field extraction is performed only if ...
+// non-zero" (:123): X[f][p(n, j)] += 1 for every flagged input n and every input j >= n flagged in the same sample (j == n is the
+// flag counter c_f[n]) -- the paper's O(E^2) intersection tracking (:117-:119), each flagged bit handled by the whole warp
+// (flag_row_update_warp scans the sample's bit-field with one load per lane).  Not inlined: keeps the copy loop at 32 registers.
+__device__ __noinline__ void account_flagged_chunks(uint32_t nz, const uint4 v, unsigned cw, unsigned frow_chunks, const uint8_t *__restrict__ foot,
+                                                    int N, int C, int f_base, int32_t *__restrict__ x)
 {
-    const long long n_pairs = (long long)n_inputs * (n_inputs + 1) / 2;
-    const int n_half = n_inputs >> 4;
+    const int lane = (int)(threadIdx.x & 31u);
+    const long long n_pairs = (long long)N * (N + 1) / 2;
+    while (nz) {
+        const int src = __ffs((int)nz) - 1;
+        nz &= nz - 1;
+        const unsigned cs = cw + (unsigned)src;
+        const unsigned dts = cs / frow_chunks, ws = cs - dts * frow_chunks;
+        const uint8_t *row_bits = foot + (size_t)dts * ((size_t)(C * N) >> 3);      // the footer bytes of time sample dts
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        uint32_t m = (q == 0) ? v.x : (q == 1) ? v.y : (q == 2) ? v.z : v.w;
-        while (m) {
-            const int b = __ffs((int)m) - 1;
-            m &= m - 1;
-            const unsigned idx = w * 128u + 32u * (unsigned)q + (unsigned)b;      // bit index inside the row
-            const int ch = (int)(idx / (unsigned)n_inputs), n = (int)(idx % (unsigned)n_inputs);
-            const uint16_t *sample = reinterpret_cast<const uint16_t *>(row_bits + (size_t)ch * (size_t)(n_inputs >> 3));
-            int32_t *x_f = x + (size_t)(f_base + ch) * (size_t)n_pairs;
-            const long long row = pair_index(n_inputs, n, n) - n;                 // p(n, j) = row + j
-            for (int k = n >> 4; k < n_half; ++k) {
-                uint32_t bits = __ldg(sample + k);
-                if (k == (n >> 4)) bits &= 0xFFFFu << (n & 15);                   // only j >= n
-                while (bits) {
-                    const int b2 = __ffs((int)bits) - 1;
-                    bits &= bits - 1;
-                    atomicAdd(x_f + row + (16 * k + b2), 1);
-                }
+        for (int q = 0; q < 4; ++q) {
+            const uint32_t mine = (q == 0) ? v.x : (q == 1) ? v.y : (q == 2) ? v.z : v.w;
+            uint32_t m = __shfl_sync(0xFFFFFFFFu, mine, src);
+            while (m) {                                              // warp-uniform
+                const int b = __ffs((int)m) - 1;
+                m &= m - 1;
+                const unsigned idx = ws * 128u + 32u * (unsigned)q + (unsigned)b;     // bit index inside the row
+                const int ch = (int)(idx / (unsigned)N), n = (int)(idx % (unsigned)N);
+                flag_row_update_warp(reinterpret_cast<const uint16_t *>(row_bits + (size_t)ch * (size_t)(N >> 3)), N, n,
+                                     x + (size_t)(f_base + ch) * (size_t)n_pairs, lane);
             }
         }
     }
@@ -163,15 +163,21 @@ __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict
             if (flags || kAccount) {
                 const uint4 *foot = reinterpret_cast<const uint4 *>(foot16);
                 uint4 *flags_v = reinterpret_cast<uint4 *>(flags + (f0 >> 3));
-                for (unsigned c = threadIdx.x; c < foot_chunks; c += blockDim.x) {
-                    const unsigned dt = c / frow_chunks, w = c - dt * frow_chunks;
-                    const uint4 v = __ldg(foot + c);
-                    if (flags) flags_v[dt * (frame_row_stride >> 3) + w] = v;
+                // the footer of a position is one warp's job, and the job rotates among the CTA's warps from position to position
+                // (the warps run through the position loop independently, so the flag work spreads over all of them)
+                const unsigned lane = threadIdx.x & 31u, n_warps = blockDim.x >> 5;
+                const unsigned duty = ((threadIdx.x >> 5) + n_warps - (pos / gridDim.x) % n_warps) % n_warps;   // 0 for this position's warp
+                for (unsigned cw = duty * 32u; cw < foot_chunks; cw += 32u * n_warps) {     // warp-uniform loop
+                    const unsigned c = cw + lane;
+                    uint4 v = make_uint4(0, 0, 0, 0);
+                    if (c < foot_chunks) {
+                        const unsigned dt = c / frow_chunks, w = c - dt * frow_chunks;
+                        v = __ldg(foot + c);
+                        if (flags) flags_v[dt * (frame_row_stride >> 3) + w] = v;
+                    }
                     if constexpr (kAccount) {
-                        // "read initially as 32-bit integers, and bit-field extraction is performed only if ... non-zero" (:123)
-                        if (v.x | v.y | v.z | v.w)
-                            account_flag_chunk(v, reinterpret_cast<const uint8_t *>(foot) + (size_t)dt * ((size_t)(C * N) >> 3), w, N,
-                                               C * (int)stream, x);
+                        const uint32_t nz = __ballot_sync(0xFFFFFFFFu, (v.x | v.y | v.z | v.w) != 0);
+                        if (nz) account_flagged_chunks(nz, v, cw, frow_chunks, reinterpret_cast<const uint8_t *>(foot), N, C, C * (int)stream, x);
                     }
                 }
             }

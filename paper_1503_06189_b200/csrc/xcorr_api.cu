@@ -651,6 +651,7 @@ struct xcorr_assembler {
                                    // two tables alternate from call to call (assemble_kernel.cuh)
     unsigned long long calls = 0;
     uint32_t *counts = nullptr;    // device uint32[8], see assemble_kernel.cuh
+    int ctas_per_sm[2] = {8, 8};   // resident CTAs of assemble_kernel<false> / <true> per SM: the grid-stride grid is exactly one wave
     uint64_t launches = 0;
     int last_cuda_error = 0;
 };
@@ -692,6 +693,13 @@ extern "C" int xcorr_assembler_create(int n_inputs, int n_freq, int t_per_frame,
     a->sh.n_streams = n_freq / C; a->sh.n_blocks = t_per_frame / S;
     const unsigned long long pay = (unsigned long long)S * C * n_inputs;
     a->sh.packet_bytes = kPacketHeaderBytes + pay + pay / 8;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a->ctas_per_sm[0], assemble_kernel<false>, 256, 0) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a->ctas_per_sm[1], assemble_kernel<true>, 256, 0) != cudaSuccess ||
+        a->ctas_per_sm[0] < 1 || a->ctas_per_sm[1] < 1) {
+        cudaGetLastError();
+        delete a;
+        return XCORR_ECUDA;
+    }
     const unsigned long long n_pos = (unsigned long long)a->sh.n_streams * (unsigned long long)a->sh.n_blocks;
     if (n_pos == 0 || n_pos > 0x7FFFFFFFull) { delete a; return XCORR_EINVAL; }
     a->n_positions = (unsigned)n_pos;
@@ -739,8 +747,8 @@ static int assemble_common(xcorr_assembler *a, xcorr_handle *h, const void *pack
         XC_CUDA(a, cudaGetLastError());
         a->launches += 1;
     }
-    // grid-stride over the positions: 8 resident CTAs of 256 threads per SM
-    unsigned blocks = (unsigned)a->n_sms * 8u;
+    // grid-stride over the positions: exactly one wave of resident CTAs (256 threads each)
+    unsigned blocks = (unsigned)a->n_sms * (unsigned)a->ctas_per_sm[h ? 1 : 0];
     if (blocks > a->n_positions) blocks = a->n_positions;
     if (h)
         assemble_kernel<true><<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, owner, owner_next, (uint8_t *)frame_dev, flags_dev,
