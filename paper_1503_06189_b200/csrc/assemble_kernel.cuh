@@ -77,11 +77,11 @@ __device__ __forceinline__ uint32_t spread4(uint32_t x) { return (((x & 0xFu) * 
 
 // kAccount, the rare path: some lanes of the warp hold footer chunks (16 bytes = 128 flag bits each, chunk cw + lane of the
 // position) with flags set (mask nz).  "read initially as 32-bit integers, and bit-field extraction is performed only if ...
-// non-zero" (:123): X[f][p(n, j)] += 1 for every flagged input n and every input j >= n flagged in the same sample (j == n is the
-// flag counter c_f[n]) -- the paper's O(E^2) intersection tracking (:117-:119), each flagged bit handled by the whole warp
+// non-zero" (:123): c_f[n] += 1 for every flagged input n and X[f][p(n, j)] += 1 for every input j > n flagged in the same
+// sample -- the paper's O(E^2) intersection tracking (:117-:119), each flagged bit handled by the whole warp
 // (flag_row_update_warp scans the sample's bit-field with one load per lane).  Not inlined: keeps the copy loop at 32 registers.
 __device__ __noinline__ void account_flagged_chunks(uint32_t nz, const uint4 v, unsigned cw, unsigned frow_chunks, const uint8_t *__restrict__ foot,
-                                                    int N, int C, int f_base, int32_t *__restrict__ x)
+                                                    int N, int C, int f_base, int32_t *__restrict__ x, int32_t *__restrict__ cnt)
 {
     const int lane = (int)(threadIdx.x & 31u);
     const long long n_pairs = (long long)N * (N + 1) / 2;
@@ -101,20 +101,21 @@ __device__ __noinline__ void account_flagged_chunks(uint32_t nz, const uint4 v, 
                 const unsigned idx = ws * 128u + 32u * (unsigned)q + (unsigned)b;     // bit index inside the row
                 const int ch = (int)(idx / (unsigned)N), n = (int)(idx % (unsigned)N);
                 flag_row_update_warp(reinterpret_cast<const uint16_t *>(row_bits + (size_t)ch * (size_t)(N >> 3)), N, n,
-                                     x + (size_t)(f_base + ch) * (size_t)n_pairs, lane);
+                                     x + (size_t)(f_base + ch) * (size_t)n_pairs, cnt + (size_t)(f_base + ch) * (size_t)N, lane);
             }
         }
     }
 }
 
 // kAccount = false: xcorr_assemble.  kAccount = true: xcorr_assemble_accounted -- `x` = the handle's intersection / counter
-// accumulator int32[F][P], `lost_acc` = its per-channel loss counters (both added to).
+// accumulator int32[F][P], `cnt` = its flag counters int32[F][N], `lost_acc` = its per-channel loss counters (all added to).
 template <bool kAccount>
-__global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict__ packets, AssembleShape sh,
+__global__ void __launch_bounds__(256, 6) assemble_kernel(const uint8_t *__restrict__ packets, AssembleShape sh,
                                                         const uint32_t *__restrict__ owner, uint32_t *__restrict__ owner_next,
                                                         uint8_t *__restrict__ frame,
                                                         uint8_t *__restrict__ flags, int32_t *__restrict__ lost, uint32_t *__restrict__ counts,
-                                                        uint32_t *__restrict__ counts_out, int32_t *__restrict__ x, int32_t *__restrict__ lost_acc)
+                                                        uint32_t *__restrict__ counts_out, int32_t *__restrict__ x, int32_t *__restrict__ cnt,
+                                                        int32_t *__restrict__ lost_acc)
 {
     const int N = sh.n_inputs, F = sh.n_freq, S = sh.s_per_packet, C = sh.c_per_packet;
     const unsigned row_chunks = (unsigned)(C * N) >> 4;            // 16-byte vectors per time sample of one stream
@@ -177,7 +178,7 @@ __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict
                     }
                     if constexpr (kAccount) {
                         const uint32_t nz = __ballot_sync(0xFFFFFFFFu, (v.x | v.y | v.z | v.w) != 0);
-                        if (nz) account_flagged_chunks(nz, v, cw, frow_chunks, reinterpret_cast<const uint8_t *>(foot), N, C, C * (int)stream, x);
+                        if (nz) account_flagged_chunks(nz, v, cw, frow_chunks, reinterpret_cast<const uint8_t *>(foot), N, C, C * (int)stream, x, cnt);
                     }
                 }
             }
@@ -221,23 +222,12 @@ __global__ void __launch_bounds__(256) assemble_kernel(const uint8_t *__restrict
     }
 }
 
-// lost-sample counters of one frame, device -> the handle's device accumulator (xcorr_norm_process_dev)
-__global__ void lost_add_kernel(const int32_t *__restrict__ lost_frame, int32_t *__restrict__ lost_acc, int n_freq)
+// lost-sample counters (one frame's, or the host-side tallies of an integration) -> the handle's device accumulator
+// (xcorr_norm_process_dev, xcorr_read_normalized).  `src` may be device memory or page-locked host memory read in place.
+__global__ void lost_add_kernel(const int32_t *__restrict__ src, int32_t *__restrict__ lost_acc, int n_freq)
 {
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
-    if (f < n_freq) lost_acc[f] += lost_frame[f];
-}
-
-// xcorr_read_normalized: this integration's packet-loss counters = the host-counted snapshot (page-locked, read in place)
-// + the device-counted ones, which start again from zero
-__global__ void lost_gather_kernel(const int32_t *__restrict__ snapshot_host, int32_t *__restrict__ lost_acc, int32_t *__restrict__ lost_out,
-                                   int n_freq)
-{
-    const int f = blockIdx.x * blockDim.x + threadIdx.x;
-    if (f < n_freq) {
-        lost_out[f] = snapshot_host[f] + lost_acc[f];
-        lost_acc[f] = 0;
-    }
+    if (f < n_freq) lost_acc[f] += src[f];
 }
 
 }  // namespace xc

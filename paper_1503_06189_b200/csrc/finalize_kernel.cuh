@@ -38,11 +38,16 @@ __device__ __forceinline__ uint4 slot_sum_v4(const int32_t *__restrict__ acc, in
     return s;
 }
 
-// Lost-sample normalisation fused into the write (normalise_kernel.cuh): inputs of the kNormalise variant
+// Lost-sample normalisation fused into the write (normalise_kernel.cuh): inputs of the kNormalise variant.
+// The flag counters and the loss counters are double-buffered by integration: this read uses one half and, on its way, puts
+// the OTHER half (read by the previous integration's finalize pass, which stream order has completed) back to zero -- so
+// xcorr_read_normalized is this one kernel: no gather before it, no clearing pass after it.
 struct NormParams {
-    int32_t *x;              // device int32[F][P]: flag intersections, diagonal = flag counters; the intersections are
-                             // cleared here as they are read (each by exactly one thread), the diagonal by clear_diag_kernel
-    const int32_t *lost;     // device int32[F]: time samples lost with their packets, per channel
+    int32_t *x;              // device int32[F][P]: flag intersections (i < j); cleared here as they are read (each by exactly one thread)
+    const int32_t *cnt;      // device int32[F][N]: flag counters c_f[n] of this integration
+    int32_t *cnt_clear;      // device int32[F][N]: the other half, zeroed by the diagonal blocks
+    const int32_t *lost;     // device int32[F]: time samples lost with their packets, per channel, this integration
+    int32_t *lost_clear;     // device int32[F]: the other half, zeroed by block (0, 0, f)
     int32_t *lost_out;       // device int32[F][P] or nullptr: the normalisation matrix L itself
     uint32_t n_samples;      // T: samples integrated since the last read
 };
@@ -64,7 +69,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
     __shared__ uint32_t sQ[32][33];   // [col][row]
     __shared__ uint32_t sX[32][33];   // [row j][col i] of the transposed patch (diagonal super-tiles only)
     __shared__ uint32_t sS[4][32];    // column sums: [0] sh_i [1] sl_i (rows of the patch)  [2] sh_j [3] sl_j (columns)
-    __shared__ int32_t sC[2][32];     // kNormalise: flag counters c_f[i] of the patch's rows [0] and columns [1] (the diagonal of X)
+    __shared__ int32_t sC[2][32];     // kNormalise: flag counters c_f[i] of the patch's rows [0] and columns [1]
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;   // ty in 0..7
     const int nb = n_super(n_inputs), nst = n_supertiles(nb);
     const int i0 = bi * 32, j0 = bj * 32;
@@ -89,12 +94,14 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
             sX[tx][4 * ty + 0] = vx.x; sX[tx][4 * ty + 1] = vx.y; sX[tx][4 * ty + 2] = vx.z; sX[tx][4 * ty + 3] = vx.w;
         }
         if constexpr (kNormalise) {
-            // the counters sit on the diagonal of X, one cache line each: fetch them here, beside the slot loads, once per block
+            // the counters of the patch's rows and columns: two coalesced 128-byte loads per block, beside the slot loads
             if (ty >= 4 && ty < 6) {
                 const int nn = ((ty == 4) ? i0 : j0) + tx;
-                const long long PP = (long long)n_inputs * (n_inputs + 1) / 2;
-                sC[ty - 4][tx] = (nn < n_inputs) ? np.x[(long long)f * PP + pair_index(n_inputs, nn, nn)] : 0;
+                sC[ty - 4][tx] = (nn < n_inputs) ? np.cnt[(size_t)f * n_inputs + nn] : 0;
             }
+            // the other half of the double-buffered counters goes back to zero (see NormParams)
+            if (bi == bj && ty == 6 && i0 + tx < n_inputs) np.cnt_clear[(size_t)f * n_inputs + i0 + tx] = 0;
+            if (bi == 0 && bj == 0 && threadIdx.x == 255) np.lost_clear[f] = 0;
         }
         if (ty < 4) {
             // ty 0,1: sh, sl of row input i0 + tx (A block of its CTA half); ty 2,3: of column input j0 + tx
@@ -112,9 +119,12 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
     const long long P = (long long)n_inputs * (n_inputs + 1) / 2;
     const uint32_t shj = sS[2][tx], slj = sS[3][tx];
     int32_t x_jj = 0, lost_f = 0;
+    float scale_f = 0.0f;             // the scale of a pair neither of whose inputs was ever flagged: the packet loss alone
     if constexpr (kNormalise) {
         x_jj = sC[1][tx];
         lost_f = np.lost[f];
+        const int32_t valid_f = (int32_t)np.n_samples - lost_f;
+        scale_f = (valid_f > 0) ? __fdiv_rn((float)np.n_samples, (float)valid_f) : 0.0f;
     }
     for (int ic = ty; ic < 32; ic += 8) {
         const int i = i0 + ic, j = j0 + tx;
@@ -138,8 +148,11 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
                     if (x_ij) np.x[p] = 0;             // ends the integration: this thread is the only reader of X[p]
                 }
                 const int32_t lost_ij = lost_f + x_ii + ((i != j) ? (x_jj - x_ij) : 0);
-                const int32_t valid = (int32_t)np.n_samples - lost_ij;
-                const float scale = (valid > 0) ? __fdiv_rn((float)np.n_samples, (float)valid) : 0.0f;
+                float scale = scale_f;
+                if (lost_ij != lost_f) {               // same expression, evaluated only where a flag counter comes in
+                    const int32_t valid = (int32_t)np.n_samples - lost_ij;
+                    scale = (valid > 0) ? __fdiv_rn((float)np.n_samples, (float)valid) : 0.0f;
+                }
                 *reinterpret_cast<float2 *>(reinterpret_cast<float *>(out_v) + p * 2) =
                     make_float2(__fmul_rn((float)(int32_t)re, scale), __fmul_rn((float)(int32_t)im, scale));
                 if (np.lost_out) np.lost_out[p] = lost_ij;
@@ -148,15 +161,6 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
             }
         }
     }
-}
-
-// after finalize_kernel<true>: flag counters (the diagonal of X) back to zero.  One thread per (f, input).
-__global__ void __launch_bounds__(256) clear_diag_kernel(int32_t *__restrict__ x, int n_inputs, int n_freq)
-{
-    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= (long long)n_inputs * n_freq) return;
-    const int f = (int)(k / n_inputs), n = (int)(k % n_inputs);
-    x[(long long)f * ((long long)n_inputs * (n_inputs + 1) / 2) + pair_index(n_inputs, n, n)] = 0;
 }
 
 }  // namespace xc

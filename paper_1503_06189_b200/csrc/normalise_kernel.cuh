@@ -28,10 +28,11 @@
 
 namespace xc {
 
-// One flagged bit (sample s, input n), handled by a whole warp: add 1 to X[f][p(n, j)] for every input j >= n flagged in
-// the same sample (j == n gives the counter c_f[n] on the diagonal).  The sample's bit-field is n_inputs / 16 aligned
-// halfwords; lane l takes halfwords (n >> 4) + l, + 32, ... so the row is scanned with one (L1-resident) load per lane.
-__device__ __forceinline__ void flag_row_update_warp(const uint16_t *__restrict__ sample_bits, int n_inputs, int n, int32_t *x_f, int lane)
+// One flagged bit (sample s, input n), handled by a whole warp: add 1 to the counter c_f[n] and to X[f][p(n, j)] for every
+// input j > n flagged in the same sample.  The sample's bit-field is n_inputs / 16 aligned halfwords; lane l takes halfwords
+// (n >> 4) + l, + 32, ... so the row is scanned with one (L1-resident) load per lane.
+__device__ __forceinline__ void flag_row_update_warp(const uint16_t *__restrict__ sample_bits, int n_inputs, int n, int32_t *x_f,
+                                                     int32_t *cnt_f, int lane)
 {
     const int n_half = n_inputs >> 4;
     const long long row = pair_index(n_inputs, n, n) - n;     // p(n, j) = row + j
@@ -41,7 +42,8 @@ __device__ __forceinline__ void flag_row_update_warp(const uint16_t *__restrict_
         while (w) {
             const int b = __ffs((int)w) - 1;
             w &= w - 1;
-            atomicAdd(x_f + row + (16 * k + b), 1);
+            const int j = 16 * k + b;
+            atomicAdd(j == n ? cnt_f + n : x_f + row + j, 1);
         }
     }
 }
@@ -63,7 +65,7 @@ constexpr int kFlagUnroll = 4;   // 16-byte chunks per lane and iteration: 2 KiB
 
 // warp-stride over 2 KiB pieces of the bit-field; n_bytes = T * F * N / 8
 __global__ void __launch_bounds__(256) flag_count_kernel(const uint8_t *__restrict__ flags, unsigned long long n_bytes, int n_inputs,
-                                                          int n_freq, int32_t *__restrict__ x)
+                                                          int n_freq, int32_t *__restrict__ x, int32_t *__restrict__ cnt)
 {
     const int lane = threadIdx.x & 31;
     const unsigned long long warp = ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -107,7 +109,7 @@ __global__ void __launch_bounds__(256) flag_count_kernel(const uint8_t *__restri
                         const int n = (int)(rel - ds * (uint32_t)n_inputs);
                         const int f = (int)((f_first + ds) % (uint32_t)n_freq);
                         flag_row_update_warp(reinterpret_cast<const uint16_t *>(flags + (s_first + ds) * sample_bytes), n_inputs, n,
-                                             x + (size_t)f * n_pairs, lane);
+                                             x + (size_t)f * n_pairs, cnt + (size_t)f * n_inputs, lane);
                     }
                 }
             }

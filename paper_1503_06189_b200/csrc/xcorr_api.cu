@@ -53,14 +53,16 @@ struct xcorr_handle {
     PFN_encodeTiled encode = nullptr;
     // lost-sample normalisation (xcorr_norm_enable): flag-intersection accumulator, packet-loss counters
     bool norm = false;
-    int32_t *flag_x = nullptr;       // device int32[F][P]
-    int32_t *lost_dev_acc = nullptr; // device int32[F]: counters added on the device (xcorr_norm_process_dev)
+    int32_t *flag_x = nullptr;       // device int32[F][P]: flag intersections (i < j)
+    int32_t *flag_cnt = nullptr;     // device int32[2][F][N]: flag counters, double-buffered by integration (finalize_kernel.cuh)
+    int32_t *lost_dev_acc = nullptr; // device int32[2][F]: packet-loss counters, double-buffered the same way
+    int norm_half = 0;               // the half the current integration counts into
     bool lost_dev_dirty = false;
-    int32_t *lost_dev = nullptr;     // device int32[F]: this integration's counters as finalize_kernel<true> reads them
-    int32_t *lost_pinned = nullptr;  // page-locked, device-mapped int32[2][F]: snapshots of lost_acc that lost_gather_kernel
-                                     // reads in place (no copy-engine operation in the stream); read r uses half r % 2
+    int32_t *lost_pinned = nullptr;  // page-locked, device-mapped int32[2][F]: snapshots of lost_acc that lost_add_kernel
+                                     // reads in place (no copy-engine operation in the stream); snapshot r uses half r % 2
     unsigned long long norm_reads = 0;
-    long long *lost_acc = nullptr;   // host: lost samples per channel since the last read
+    long long *lost_acc = nullptr;   // host: lost samples per channel since the last read (xcorr_norm_process)
+    bool lost_host_dirty = false;    // lost_acc holds counts of the current integration
     int32_t *staging_lost = nullptr; // device int32[F][P] for host reads of the normalisation matrix
     cudaEvent_t lost_used[2] = {nullptr, nullptr};   // recorded after the finalize launch that read the snapshot half
     bool flags_dirty = false;        // flag_x holds counts of the current integration
@@ -173,7 +175,7 @@ extern "C" void xcorr_destroy(xcorr_handle *h)
     cudaFree(h->tile_slot_begin);
     cudaFree(h->flag_x);
     cudaFree(h->lost_dev_acc);
-    cudaFree(h->lost_dev);
+    cudaFree(h->flag_cnt);
     cudaFree(h->staging_lost);
     if (h->lost_pinned) cudaFreeHost(h->lost_pinned);
     if (h->order_event) cudaEventDestroy(h->order_event);
@@ -354,22 +356,26 @@ static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *
         XC_CUDA(h, cudaMemsetAsync(h->sums, 0, h->sums_bytes, s));
     }
     NormParams np = {};
-    int lost_half = 0;
     if (normalise) {
-        // packet-loss counters: host accumulator -> page-locked snapshot the kernel reads in place; a half is reused two
-        // reads later, after the event recorded behind its reader
-        lost_half = (int)(h->norm_reads++ & 1u);
-        XC_CUDA(h, cudaEventSynchronize(h->lost_used[lost_half]));
-        int32_t *snap = h->lost_pinned + (size_t)lost_half * h->n_freq;
-        for (int f = 0; f < h->n_freq; ++f) snap[f] = (int32_t)h->lost_acc[f];
-        // lost_dev = host-counted snapshot + device-counted counters (xcorr_norm_process_dev), the latter cleared for the next integration
-        lost_gather_kernel<<<(h->n_freq + 255) / 256, 256, 0, s>>>(snap, h->lost_dev_acc, h->lost_dev, h->n_freq);
-        XC_CUDA(h, cudaGetLastError());
-        h->launches += 1;
-        XC_CUDA(h, cudaEventRecord(h->lost_used[lost_half], s));
-        h->lost_dev_dirty = false;
-        np.lost = h->lost_dev;
+        const size_t cnt_half = (size_t)h->n_freq * h->n_inputs;
+        int32_t *lost_cur = h->lost_dev_acc + (size_t)h->norm_half * h->n_freq;
+        if (h->lost_host_dirty) {
+            // packet-loss counters tallied on the host (xcorr_norm_process): a page-locked snapshot the device adds in place; a
+            // snapshot half is reused two such reads later, after the event recorded behind its reader
+            const int snap_half = (int)(h->norm_reads++ & 1u);
+            XC_CUDA(h, cudaEventSynchronize(h->lost_used[snap_half]));
+            int32_t *snap = h->lost_pinned + (size_t)snap_half * h->n_freq;
+            for (int f = 0; f < h->n_freq; ++f) snap[f] = (int32_t)h->lost_acc[f];
+            lost_add_kernel<<<(h->n_freq + 255) / 256, 256, 0, s>>>(snap, lost_cur, h->n_freq);
+            XC_CUDA(h, cudaGetLastError());
+            h->launches += 1;
+            XC_CUDA(h, cudaEventRecord(h->lost_used[snap_half], s));
+        }
         np.x = h->flag_x;
+        np.cnt = h->flag_cnt + (size_t)h->norm_half * cnt_half;
+        np.cnt_clear = h->flag_cnt + (size_t)(h->norm_half ^ 1) * cnt_half;
+        np.lost = lost_cur;
+        np.lost_clear = h->lost_dev_acc + (size_t)(h->norm_half ^ 1) * h->n_freq;
         np.lost_out = lost_dst;
         np.n_samples = (uint32_t)h->samples_since_read;
     }
@@ -397,20 +403,24 @@ static int read_common(xcorr_handle *h, void *vis_out, bool normalise, int32_t *
     h->offset_samples = 0;
     h->clean = true;
     if (h->norm) {   // the flag / loss state belongs to the integration that just ended
-        if (h->flags_dirty) {
-            if (normalise) {   // finalize_kernel<true> has already cleared the intersections it read; the counters remain
-                const long long nd = (long long)h->n_inputs * h->n_freq;
-                clear_diag_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, s>>>(h->flag_x, h->n_inputs, h->n_freq);
-                XC_CUDA(h, cudaGetLastError());
-                h->launches += 1;
-            } else {
+        if (normalise) {
+            // finalize_kernel<true> has cleared the intersections it read and the OTHER half of the counters: that half is the
+            // next integration's
+            h->norm_half ^= 1;
+        } else {
+            const size_t cnt_half = (size_t)h->n_freq * h->n_inputs;
+            if (h->flags_dirty) {
                 XC_CUDA(h, cudaMemsetAsync(h->flag_x, 0, lost_matrix_bytes, s));
+                XC_CUDA(h, cudaMemsetAsync(h->flag_cnt + (size_t)h->norm_half * cnt_half, 0, sizeof(int32_t) * cnt_half, s));
             }
+            if (h->lost_dev_dirty)
+                XC_CUDA(h, cudaMemsetAsync(h->lost_dev_acc + (size_t)h->norm_half * h->n_freq, 0, sizeof(int32_t) * h->n_freq, s));
         }
         h->flags_dirty = false;
-        if (h->lost_dev_dirty) XC_CUDA(h, cudaMemsetAsync(h->lost_dev_acc, 0, sizeof(int32_t) * h->n_freq, s));
         h->lost_dev_dirty = false;
-        for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] = 0;
+        if (h->lost_host_dirty)
+            for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] = 0;
+        h->lost_host_dirty = false;
     }
     if (!on_device) XC_CUDA(h, cudaMemcpyAsync(vis_out, h->staging, h->output_bytes, cudaMemcpyDeviceToHost, s));
     if (lost_matrix_out && !lost_on_device)
@@ -448,7 +458,7 @@ extern "C" int xcorr_norm_enable(xcorr_handle *h)
         if (e != cudaSuccess) { h->last_cuda_error = (int)e; cudaGetLastError(); }
         cudaFree(h->flag_x); h->flag_x = nullptr;
         cudaFree(h->staging_lost); h->staging_lost = nullptr;
-        cudaFree(h->lost_dev); h->lost_dev = nullptr;
+        cudaFree(h->flag_cnt); h->flag_cnt = nullptr;
         cudaFree(h->lost_dev_acc); h->lost_dev_acc = nullptr;
         if (h->lost_pinned) cudaFreeHost(h->lost_pinned);
         h->lost_pinned = nullptr;
@@ -462,15 +472,18 @@ extern "C" int xcorr_norm_enable(xcorr_handle *h)
     cudaError_t e;
     if ((e = cudaMalloc(&h->flag_x, lost_matrix_bytes)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
     if ((e = cudaMalloc(&h->staging_lost, lost_matrix_bytes)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
-    if ((e = cudaMalloc(&h->lost_dev, sizeof(int32_t) * h->n_freq)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
-    if ((e = cudaMalloc(&h->lost_dev_acc, sizeof(int32_t) * h->n_freq)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
+    const size_t cnt_bytes = sizeof(int32_t) * 2 * (size_t)h->n_freq * h->n_inputs;
+    if ((e = cudaMalloc(&h->flag_cnt, cnt_bytes)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
+    if ((e = cudaMalloc(&h->lost_dev_acc, sizeof(int32_t) * 2 * h->n_freq)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
     if ((e = cudaMallocHost(&h->lost_pinned, sizeof(int32_t) * 2 * h->n_freq)) != cudaSuccess) return undo(XCORR_ENOMEM, e);
     h->lost_acc = new (std::nothrow) long long[h->n_freq]();
     if (!h->lost_acc) return undo(XCORR_ENOMEM, cudaSuccess);
     for (int k = 0; k < 2; ++k)
         if ((e = cudaEventCreateWithFlags(&h->lost_used[k], cudaEventDisableTiming)) != cudaSuccess) return undo(XCORR_ECUDA, e);
     if ((e = cudaMemset(h->flag_x, 0, lost_matrix_bytes)) != cudaSuccess) return undo(XCORR_ECUDA, e);
-    if ((e = cudaMemset(h->lost_dev_acc, 0, sizeof(int32_t) * h->n_freq)) != cudaSuccess) return undo(XCORR_ECUDA, e);
+    if ((e = cudaMemset(h->flag_cnt, 0, cnt_bytes)) != cudaSuccess) return undo(XCORR_ECUDA, e);
+    if ((e = cudaMemset(h->lost_dev_acc, 0, sizeof(int32_t) * 2 * h->n_freq)) != cudaSuccess) return undo(XCORR_ECUDA, e);
+    h->norm_half = 0;
     h->norm = true;
     return XCORR_OK;
 }
@@ -485,7 +498,8 @@ extern "C" int xcorr_norm_process_dev(xcorr_handle *h, const uint8_t *flags_dev,
     if (rc != XCORR_OK) return rc;
     if ((flags_dev || lost_samples_dev) && (rc = order_after_previous(h, (cudaStream_t)cuda_stream)) != XCORR_OK) return rc;
     if (lost_samples_dev) {
-        lost_add_kernel<<<(h->n_freq + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(lost_samples_dev, h->lost_dev_acc, h->n_freq);
+        lost_add_kernel<<<(h->n_freq + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(lost_samples_dev, h->lost_dev_acc + (size_t)h->norm_half * h->n_freq,
+                                                                                        h->n_freq);
         XC_CUDA(h, cudaGetLastError());
         h->launches += 1;
         h->lost_dev_dirty = true;
@@ -501,6 +515,7 @@ extern "C" int xcorr_norm_process(xcorr_handle *h, const uint8_t *flags_dev, con
         for (int f = 0; f < h->n_freq; ++f)
             if (lost_samples_host[f] < 0 || lost_samples_host[f] > h->n_time) return XCORR_EINVAL;
         for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] += lost_samples_host[f];
+        h->lost_host_dirty = true;
     }
     if (flags_dev) {
         int rc = check_device(h->device);
@@ -517,7 +532,8 @@ static int launch_flag_count(xcorr_handle *h, const uint8_t *flags_dev, void *cu
         const unsigned long long n_pieces = (n_bytes + 16ull * 32 * kFlagUnroll - 1) / (16ull * 32 * kFlagUnroll);   // 2 KiB per warp and iteration
         int blocks = h->n_sms * 8;     // warp-stride, 8 resident CTAs of 256 threads (8 warps) per SM
         if ((unsigned long long)blocks * 8ull > n_pieces) blocks = (int)((n_pieces + 7) / 8);
-        flag_count_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>(flags_dev, n_bytes, h->n_inputs, h->n_freq, h->flag_x);
+        flag_count_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>(flags_dev, n_bytes, h->n_inputs, h->n_freq, h->flag_x,
+                                                                         h->flag_cnt + (size_t)h->norm_half * h->n_freq * h->n_inputs);
         XC_CUDA(h, cudaGetLastError());
         h->launches += 1;
         h->flags_dirty = true;
@@ -752,10 +768,12 @@ static int assemble_common(xcorr_assembler *a, xcorr_handle *h, const void *pack
     if (blocks > a->n_positions) blocks = a->n_positions;
     if (h)
         assemble_kernel<true><<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, owner, owner_next, (uint8_t *)frame_dev, flags_dev,
-                                                     lost_dev, a->counts, counts_dev, h->flag_x, h->lost_dev_acc);
+                                                     lost_dev, a->counts, counts_dev, h->flag_x,
+                                                     h->flag_cnt + (size_t)h->norm_half * h->n_freq * h->n_inputs,
+                                                     h->lost_dev_acc + (size_t)h->norm_half * h->n_freq);
     else
         assemble_kernel<false><<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, owner, owner_next, (uint8_t *)frame_dev, flags_dev,
-                                                      lost_dev, a->counts, counts_dev, nullptr, nullptr);
+                                                      lost_dev, a->counts, counts_dev, nullptr, nullptr, nullptr);
     XC_CUDA(a, cudaGetLastError());
     a->launches += 1;
     a->calls += 1;   // the tables swap roles only once both kernels are in the stream
