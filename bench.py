@@ -41,7 +41,8 @@ import workloads as wl  # noqa: E402
 NOMINAL_INT8_TOPS = 4500.0  # dense int8, B200 nominal (2x the 2.25 PFLOP/s dense bf16 figure)
 # dram__bytes_read.sum + dram__bytes_write.sum of xengine_kernel<false> for one C2 launch, from the committed
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = {"C2": 277.2e6}   # profiles/r01_ncu_full_bench_c2.md: 268.49 MB read + 8.66 MB written
+# profiles/r02_ncu_full_bench_c2.md (268.49 MB read + 11.66 MB written) and r02_ncu_full_bench_c4_c5.md
+NCU_TRAFFIC_BYTES = {"C2": 280.15e6, "C3": None, "C4": 633.7e6, "C5": 4266.9e6}
 # tcgen05 MMAs (M256 N256 K32, 2 CTAs) xengine_kernel issues per 32-sample K-step of a 256 x 256 super-tile
 MMAS_DIAG, MMAS_OFFDIAG = 2, 4
 
@@ -306,7 +307,7 @@ def tensor_roofline(cfg, k_ms, peaks, ceiling=None):
     peak_sustained = 2.0 * peaks["bf16_sustained"] if peaks.get("bf16_sustained") else None
     iou = issued_over_useful(cfg)
     r = {"bound": "tensor", "kernel": "xengine_kernel (xcorr_process)", "achieved": achieved, "peak": peak, "unit": "TOP/s",
-         "frac": achieved / peak, "kernel_ms": k_ms, "algorithmic_ops_per_launch": alg_ops,
+         "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "kernel_ms": k_ms, "algorithmic_ops_per_launch": alg_ops,
          "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
          "frac_of_sustained_peak": (achieved / peak_sustained) if peak_sustained else None, "peak_sustained": peak_sustained,
          "issued_over_useful": iou, "issued_int8_tops": achieved * iou,
@@ -464,7 +465,6 @@ def main():
     # `frac` keeps the 2 x measured bf16 burst peak as denominator (int8:bf16 nominal ratio 4.5:2.25) for continuity; the
     # measured issue ceiling of the int8 pipe itself is beside it (int8_issue_ceiling_tops, frac_*_of_issue_ceiling)
     roofline = tensor_roofline(cfg, k_ms, peaks, ceiling)
-    roofline["traffic"] = NCU_TRAFFIC_BYTES.get(cfg.name)
     roofline["kernel_ms_min"] = min(kern_ms)
     roofline["peak_source"] = f"2 x bf16_tflops (burst) of MEASURED_PEAKS.json [{peaks['source']}]; int8:bf16 nominal ratio 4.5:2.25"
     if ceiling:

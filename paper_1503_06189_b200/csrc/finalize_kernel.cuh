@@ -78,6 +78,18 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
     const int tile = f * nst + supertile_index(nb, I, J);
     const int sb = tile_slot_begin[tile], se = tile_slot_begin[tile + 1];
 
+    // kNormalise: the flag intersections X_ij of the four pairs this thread writes in phase 2 (rows i0 + ty + 8k, column j0 + tx:
+    // 128 B contiguous per warp and row) are fetched here, with the slot loads, so phase 2 has no second round of loads
+    int32_t x_pre[4] = {0, 0, 0, 0};
+    if constexpr (kNormalise) {
+        const long long PP = (long long)n_inputs * (n_inputs + 1) / 2;
+        const int j = j0 + tx;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int i = i0 + ty + 8 * k;
+            if (j < n_inputs && i < j) x_pre[k] = np.x[(long long)f * PP + pair_index(n_inputs, i, j)];
+        }
+    }
     // phase 1: thread (tx = row, ty = group of 4 columns): 16-byte loads, 512 B contiguous per warp
     {
         const int il = (i0 % kSuper) + tx;            // row inside the super-block
@@ -126,7 +138,9 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
         const int32_t valid_f = (int32_t)np.n_samples - lost_f;
         scale_f = (valid_f > 0) ? __fdiv_rn((float)np.n_samples, (float)valid_f) : 0.0f;
     }
-    for (int ic = ty; ic < 32; ic += 8) {
+#pragma unroll(kNormalise ? 4 : 1)
+    for (int k = 0; k < 4; ++k) {
+        const int ic = ty + 8 * k;
         const int i = i0 + ic, j = j0 + tx;
         if (j < n_inputs && i <= j) {
             const uint32_t shi = sS[0][ic], sli = sS[1][ic];
@@ -142,19 +156,16 @@ __global__ void __launch_bounds__(256) finalize_kernel(const int32_t *__restrict
             if constexpr (kNormalise) {
                 // L = lost + c_i + c_j - X_ij (the point (i, i) receives its counter once); V~ = V * T / (T - L)
                 const int32_t x_ii = sC[0][ic];
-                int32_t x_ij = 0;
-                if (i != j && x_ii != 0 && x_jj != 0) {   // two inputs are flagged together at most as often as either one is: X_ij <= min(c_i, c_j)
-                    x_ij = np.x[p];
-                    if (x_ij) np.x[p] = 0;             // ends the integration: this thread is the only reader of X[p]
-                }
+                const int32_t x_ij = x_pre[k];
+                if (x_ij) np.x[p] = 0;                 // ends the integration: this thread is the only reader of X[p]
                 const int32_t lost_ij = lost_f + x_ii + ((i != j) ? (x_jj - x_ij) : 0);
                 float scale = scale_f;
                 if (lost_ij != lost_f) {               // same expression, evaluated only where a flag counter comes in
                     const int32_t valid = (int32_t)np.n_samples - lost_ij;
                     scale = (valid > 0) ? __fdiv_rn((float)np.n_samples, (float)valid) : 0.0f;
                 }
-                *reinterpret_cast<float2 *>(reinterpret_cast<float *>(out_v) + p * 2) =
-                    make_float2(__fmul_rn((float)(int32_t)re, scale), __fmul_rn((float)(int32_t)im, scale));
+                __stcs(reinterpret_cast<float2 *>(reinterpret_cast<float *>(out_v) + p * 2),
+                       make_float2(__fmul_rn((float)(int32_t)re, scale), __fmul_rn((float)(int32_t)im, scale)));
                 if (np.lost_out) np.lost_out[p] = lost_ij;
             } else {
                 __stcs(reinterpret_cast<int2 *>(out + p * 2), make_int2((int32_t)re, (int32_t)im));
