@@ -1,15 +1,18 @@
 // schedule.hpp -- host-side work decomposition for the persistent X-engine kernel (pure C++, no CUDA).
 //
 // Work item  = one super-tile (f, I <= J) over the whole frame; it is cut along time into STAGES of
-//              kStageT samples.  A diagonal item (I == J) costs 3 MMAs per 32-sample K-step, an
-//              off-diagonal one 4.
+//              kStageT samples.  Cost model per stage: 11 for a diagonal item (I == J), 16 for an off-diagonal one --
+//              measured, not counted: a diagonal K-step is 2 MMAs against 4, but in the N > 256 kernel
+//              both forms are bound by the shared-memory side and the diagonal one keeps less of its advantage.  Sweep of
+//              the diagonal cost at 16 for the other (C4 / C5 xcorr_process, us): 9: 656 / 1413, 10: 646 / 1354,
+//              11: 645 / 1355, 12: 654 / 1447, 13: 658 / 1518.  N <= 256 has diagonal items only, any constant does.
 // Worker     = one CTA pair (two SMs, one 2-CTA tcgen05 MMA stream); there are `n_workers` of them.
 //
 // Hybrid data-parallel / stream-K split (integer addition is exact and order independent, so a
 // super-tile may be summed by several workers, each adding its partial into the accumulator):
-//   * the first floor(n_items / n_workers) * n_workers items go round-robin, whole, to the workers --
-//     consecutive items (same channel, neighbouring super-tiles) run at the same time on different
-//     workers, so blocks shared between them are served by L2;
+//   * whole rounds of n_workers items go round-robin, whole, to the workers, as long as that leaves no worker
+//     above the mean load of the whole job -- consecutive items (same channel, neighbouring super-tiles) run at
+//     the same time on different workers, so blocks shared between them are served by L2;
 //   * the stages of the remaining items are dealt out as contiguous runs so that every worker ends
 //     with (nearly) the same total cost ("water filling").
 // Every (item, stage) is assigned to exactly one worker (checked by tests/test_host_logic.py).
@@ -49,16 +52,34 @@ inline Schedule make_schedule(int n_inputs, int n_freq, int n_time, int n_worker
     const int nb = (n_inputs + 255) / 256;
     const int nst = nb * (nb + 1) / 2;
 
-    struct Item { int f, I, J, tile; int64_t cost_per_stage; };
+    struct Item { int f, I, J, tile; int64_t cost_per_stage; };   // cost model: see the header
     std::vector<Item> items;
     items.reserve((size_t)n_freq * nst);
     for (int f = 0; f < n_freq; ++f)
         for (int I = 0; I < nb; ++I)
             for (int J = I; J < nb; ++J)
-                items.push_back({f, I, J, f * nst + (I * (2 * nb - I + 1) / 2 + (J - I)), I == J ? 3 : 4});
+                items.push_back({f, I, J, f * nst + (I * (2 * nb - I + 1) / 2 + (J - I)), I == J ? 11 : 16});
 
     const int64_t n_items = (int64_t)items.size();
-    const int64_t n_dp = (n_items / n_workers) * n_workers;
+    // whole rounds of n_workers items go data-parallel only as long as no worker ends above the mean load of the whole job
+    // (2 % slack): an item dearer than the mean (N = 512, T long: one off-diagonal item per worker is 8192 of a mean of 7085)
+    // has to be cut, so there the water filling takes everything
+    int64_t total_cost = 0;
+    for (const Item &it : items) total_cost += it.cost_per_stage * s.n_stages;
+    const int64_t cap = total_cost / n_workers + total_cost / n_workers / 50 + 4;
+    int64_t n_dp = 0;
+    {
+        std::vector<int64_t> trial(n_workers, 0);
+        for (int64_t r = 0; (r + 1) * n_workers <= n_items; ++r) {
+            int64_t mx = 0;
+            for (int w = 0; w < n_workers; ++w) {
+                trial[w] += items[r * n_workers + w].cost_per_stage * s.n_stages;
+                mx = std::max(mx, trial[w]);
+            }
+            if (mx > cap) break;
+            n_dp = (r + 1) * n_workers;
+        }
+    }
     std::vector<std::vector<Segment>> per(n_workers);
     std::vector<int64_t> load(n_workers, 0);
 
