@@ -32,6 +32,27 @@ def test_symbol_exported(name):
     assert getattr(L, name) is not None
 
 
+def test_library_exports_only_the_declared_c_abi():
+    """libxcorr.so carries no test scaffolding and no measurement code: every extern "C" symbol it exports is declared in
+    include/*.h (the SIMT second opinion lives in tests/support, the int8 issue probe in libxcorr_probe.so)."""
+    import subprocess
+    from paper_1503_06189_b200 import _build
+    xb.lib()
+    out = subprocess.run(["nm", "-D", "--defined-only", str(_build.LIB)], capture_output=True, text=True, check=True).stdout
+    exported = {ln.split()[-1] for ln in out.splitlines() if ln.split() and not ln.split()[-1].startswith("_")}
+    c_abi = {name for name in exported if name.startswith("xcorr_")}
+    assert c_abi == set(_declared_symbols())
+    assert not any("simt" in name.lower() or "probe" in name.lower() or "profile" in name.lower() for name in exported)
+
+
+def test_support_libraries_build_and_export():
+    """The two non-product libraries build for sm_100a without a GPU and export their one entry point each."""
+    from paper_1503_06189_b200 import probe
+    from tests import support
+    assert probe.lib().xcorr_probe_int8_issue is not None
+    assert support.lib().simt_xcorr is not None
+
+
 def test_no_torch_types_in_abi():
     for h in INCLUDE.glob("*.h"):
         code = re.sub(r"/\*.*?\*/", "", h.read_text(), flags=re.S)   # comments may mention torch pin_memory
@@ -46,10 +67,21 @@ def test_strerror_is_total():
     assert "overflow" in xb.xcorr_strerror(xb.XCORR_EOVERFLOW)
 
 
-@pytest.mark.parametrize("shape", [(0, 4, 16), (16, 0, 16), (16, 4, 0), (-16, 4, 16), (24, 4, 16), (8, 1, 1), (250, 2, 64)])
+@pytest.mark.parametrize("shape", [(0, 4, 16), (16, 0, 16), (16, 4, 0), (-16, 4, 16), (24, 4, 16), (8, 1, 1), (250, 2, 64),
+                                   # shapes whose work tables alone would not fit: refused before any schedule is built
+                                   (65536, 65535, 16), (65536, 9, 16), (4096, 2049, 16)])
 def test_create_rejects_bad_shapes_without_touching_the_gpu(shape):
     rc, h = xb.xcorr_create(*shape)
     assert rc == xb.XCORR_EINVAL and h == 0
+
+
+def test_schedule_of_an_oversized_shape_is_refused_not_attempted():
+    with pytest.raises(xb.XCorrError):
+        xb.xcorr_debug_schedule(65536, 65535, 16, 74)
+    with pytest.raises(xb.XCorrError):
+        xb.xcorr_debug_schedule(4096, 2048, 64, 74)                 # 2048 channels x 136 super-tiles = 278,528 > 2^18 work items
+    seg, wb = xb.xcorr_debug_schedule(4096, 1927, 64, 74)           # 262,072 work items: the largest that is still scheduled
+    assert len(seg) >= 262072 and wb[-1] == len(seg)
 
 
 def test_null_handles_are_harmless():
