@@ -86,9 +86,12 @@ struct KernelCfg {
     // by the same group -- kPackedStages is a multiple of kUnpackGroups (with 3 slots and 2 groups a group could reach its
     // next use of a slot while the other group's load into that slot was still in flight, pass the wait on the stale
     // parity and unpack old bytes: seen as wrong visibilities on C5).  Plane ring (unpack -> MMA -> unpack): its phases
-    // complete through tcgen05.commit, in issue order, and a group has itself waited for the commit of the stage after the
-    // one in question before it comes back to a slot, so an odd ring is sound there.
+    // complete through tcgen05.commit, in issue order.  A group at stage `it` waits for commit(it - ring) and would pass
+    // wrongly only if commit(it - 2 ring) were still outstanding; at its previous stage it - groups it waited for
+    // commit(it - groups - ring), which is at or after commit(it - 2 ring) whenever ring >= groups -- so any ring size not
+    // smaller than the group count is sound there, multiples or not.
     static_assert(kPackedStages % kUnpackGroups == 0, "a packed slot must always be consumed by the same unpack group");
+    static_assert(kPlaneStages >= kUnpackGroups, "plane ring: a group's previous wait must cover the phase before the one it waits for");
 };
 
 constexpr int kWarpTma = 0;
