@@ -109,14 +109,23 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_sample(cfg: wl.Config, seconds_hint: float = 12.0):
-    """Time the oracle, as it stands, on a bounded sample of `cfg`: a few whole channels of one frame."""
+def oracle_sample_frame(cfg: wl.Config):
+    """The bounded sample of `cfg` the oracle is timed on: a few whole channels of one frame (generated outside the timing)."""
     import oracle
     oracle.build()
     cores = oracle.threads()
     n_ch = max(1, min(cfg.n_freq, 8 * cores if cfg.n_inputs <= 256 else 1))
     t_samp = cfg.n_time if cfg.n_inputs <= 512 else min(cfg.n_time, 2048)
-    fr = wl.make_frame(cfg.kind, cfg.n_inputs, n_ch, t_samp, cfg.seed)
+    return wl.make_frame(cfg.kind, cfg.n_inputs, n_ch, t_samp, cfg.seed)
+
+
+def oracle_sample(cfg: wl.Config, fr=None):
+    """Time the oracle, as it stands, on a bounded sample of `cfg` (oracle_sample_frame)."""
+    import oracle
+    if fr is None:
+        fr = oracle_sample_frame(cfg)
+    cores = oracle.threads()
+    t_samp, n_ch = fr.shape[0], fr.shape[1]
     t0 = time.perf_counter()
     oracle.planar(fr)
     dt = time.perf_counter() - t0
@@ -234,10 +243,13 @@ def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    steps, warm = max(1, min(args.steps, 5)), max(0, min(args.warmup, 1))
+    # a step is one whole frame of the config through the oracle (C2: about 2.5 s on 16 cores): K up to 40 and W up to 3 are
+    # honoured as given, so the driver's --steps 20 --warmup 3 ends within two minutes
+    steps, warm = max(1, min(args.steps, 40)), max(0, min(args.warmup, 3))
+    fr = oracle_sample_frame(cfg)
     for _ in range(warm):
-        oracle_sample(cfg)
-    samples = [oracle_sample(cfg) for _ in range(steps)]
+        oracle_sample(cfg, fr)
+    samples = [oracle_sample(cfg, fr) for _ in range(steps)]
     best = samples[-1]
     v = statistics.mean(s["value"] for s in samples)
     ms = statistics.mean(s["seconds"] for s in samples) * 1e3
