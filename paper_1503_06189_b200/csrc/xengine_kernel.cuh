@@ -1,11 +1,13 @@
 // xengine_kernel.cuh -- the fused X-engine kernel for sm_100a (hot-path rows a1..a4).
 //
-//   a1  TMA stages packed bytes  frame[t][f][128 inputs]  as 128-byte rows (SWIZZLE_128B) into smem
-//   a2  unpack warps split each byte into int8 Re / Im planes (same swizzled 128-byte-row layout, so
-//       the unpack is purely element-wise and never looks at the swizzle).  The planes hold the OFFSET values
-//       h' = Re + 8, l' = Im + 8 in [0, 15] (layout.hpp "OFFSET OPERANDS": constant-zero upper nibbles cut the
-//       MMA datapath's switching power, and the part is power-limited); the same warps keep per-input column
-//       sums of h', l' so that xcorr_read can remove the offsets exactly
+//   a1  TMA stages packed bytes  frame[t][f][128 inputs]  as 128-byte rows (SWIZZLE_128B) into smem; the same boxes are
+//       requested into L2 kPrefetchStages stages ahead (cp.async.bulk.prefetch.tensor), so the loads pay L2 latency
+//   a2  unpack warps split each byte into int8 planes (same swizzled 128-byte-row layout, so the unpack is purely
+//       element-wise and never looks at the swizzle).  The planes hold the OFFSET values h' = Re + 8, l' = Im + 8 in
+//       [0, 15] and, per tile kind, s' = h' + l' or the complement 15 - l' (layout.hpp "OFFSET OPERANDS": constant-zero
+//       upper bits cut the MMA datapath's switching power, and the part is power-limited); the same warps keep per-input
+//       column sums of h', l' so that xcorr_read can remove the offsets exactly.  The 8 unpack warps work in groups on
+//       alternate stages (KernelCfg::kUnpackGroups)
 //   a3  one thread issues 2-CTA tcgen05.mma kind::i8 (M = 256 over the CTA pair, N = 256, K = 32) with
 //       both operands MN-major straight from those planes; int32 accumulators stay in TMEM (512 columns)
 //       for the whole time range of the work segment
