@@ -31,8 +31,9 @@
  *   - Stream order.  The device state of a handle (accumulator, flag / loss accumulators) is ordered by the streams the
  *     calls are given: calls on the SAME stream run in stream order; a call given ANOTHER stream than the handle's
  *     previous call first makes that stream wait, on the device (cudaStreamWaitEvent), for everything enqueued so far
- *     on the previous stream -- so xcorr_process on stream A followed by xcorr_read on stream B is safe and exact.  The
- *     previous stream must still exist at that point (XCORR_EINVAL if it has been destroyed).  The host-side
+ *     on the previous stream -- so xcorr_process on stream A followed by xcorr_read on stream B is safe and exact.  A
+ *     stream handed to a call must therefore stay alive until the handle's next call has returned (or the handle is
+ *     destroyed); if CUDA reports the previous stream as invalid the call returns XCORR_EINVAL.  The host-side
  *     bookkeeping (first frame of an integration, overflow guard, sample count) follows the order of the CALLS.
  *   - Nothing is allocated or freed after xcorr_create()/xcorr_stream_create() return (PAPER.md:49:
  *     "the entire application does not malloc or free any memory outside of startup and shutdown").
