@@ -20,6 +20,10 @@ __device__ __forceinline__ void cluster_sync()
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
+// the two halves separately; a relaxed arrive orders nothing by itself (pair it with explicit fences for what must be seen)
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
 // shared::cta address of `local` in CTA `rank` of this cluster, as a shared::cluster address
 __device__ __forceinline__ uint32_t mapa(uint32_t local, uint32_t rank)
 {

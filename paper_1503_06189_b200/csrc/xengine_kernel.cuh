@@ -184,9 +184,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     // cursor of the L2 prefetch: runs kPrefetchStages stages ahead of the loads through the worker's segment list
     int pf_sg = seg_begin, pf_st = 0;
     Segment pf_seg = {};
-    auto prefetch_next = [&]() {
+    auto prefetch_next = [&](bool request = true) {
         if (pf_sg >= seg_end) return;
-        tma_prefetch(pf_seg, pf_st);
+        if (request) tma_prefetch(pf_seg, pf_st);
         if (++pf_st >= pf_seg.stage_end) {
             if (++pf_sg < seg_end) { pf_seg = p.segments[pf_sg]; pf_st = pf_seg.stage_begin; }
         }
@@ -215,8 +215,8 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         // the frame may be the output of the previous kernel of the stream, which may have let this grid start early:
         // wait for it, unless the caller has promised complete frames (xcorr_promise_complete_frames)
         if (p.wait_frame) ptx::grid_dependency_wait();
-        if (pf_sg < seg_end) { pf_seg = p.segments[pf_sg]; pf_st = pf_seg.stage_begin; }
-        for (int k = 0; k < Cfg::kPrefetchStages; ++k) prefetch_next();
+        // loads first (every TMA instruction costs this lane on the order of 100 clk to issue, and the first MMA waits for the
+        // first box): the L2 prefetches of the stages behind them follow after the prologue barrier
         for (int sg = seg_begin; sg < seg_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++sg) {
             const Segment seg = p.segments[sg];
             for (int st = seg.stage_begin; st < seg.stage_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++st, ++tma_pre)
@@ -229,7 +229,11 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     }
     ptx::tc_fence_before_sync();
     __syncthreads();
-    ptx::cluster_sync();           // barriers of both CTAs initialised before any remote arrive / multicast commit
+    // barriers of both CTAs initialised before any remote arrive / multicast commit.  The arrive is RELAXED: the barrier
+    // initialisations were published by fence.mbarrier_init.release.cluster, and a releasing arrive would make every thread
+    // wait here for the frame loads already in flight (measured: 3.5-4 k clk per CTA)
+    ptx::cluster_arrive_relaxed();
+    ptx::cluster_wait();
     ptx::tc_fence_after_sync();
     // The accumulator / sum slots may still be read or written by the previous kernel of the stream (xcorr_read's
     // finalize_kernel, or the previous frame's xengine_kernel): the warps that touch them wait (griddepcontrol.wait) right
@@ -242,6 +246,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     if (warp == kWarpTma) {
         // ===================================================== a1: TMA producer (one lane)
         if (lane == 0) {
+            // L2 prefetch cursor: the stages loaded in the prologue need no request; then run kPrefetchStages ahead of the loads
+            if (pf_sg < seg_end) { pf_seg = p.segments[pf_sg]; pf_st = pf_seg.stage_begin; }
+            for (int k = 0; k < Cfg::kPrefetchStages; ++k) prefetch_next(k >= (int)tma_pre);
             uint32_t it = 0;
             for (int sg = seg_begin; sg < seg_end; ++sg) {
                 const Segment seg = p.segments[sg];
@@ -498,6 +505,16 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 // happens at the destination, nothing is loaded into the SM).  Two staging buffers per warp; lane 0 owns the
                 // bulk groups.
                 auto chunk_store = [&](int ch, const uint32_t (&v)[32]) {
+                    if (p.first_frame) {
+                        // first frame of an integration: plain stores straight from the registers -- lane = row, 16 bytes per
+                        // lane and instruction = 512 contiguous bytes of the slot per warp; no staging, no proxy fence, no bulk
+                        // group (an epilogue of 16 chunks: 8.5 k -> about 4 k clk, which is what reading TMEM costs)
+                        int32_t *dst = slot_warp + (size_t)(chunk_col(ch) >> 2) * (32 * 4) + lane * 4;
+#pragma unroll
+                        for (int g = 0; g < 8; ++g)
+                            ptx::st_global_v4(dst + g * (32 * 4), (int32_t)v[4 * g], (int32_t)v[4 * g + 1], (int32_t)v[4 * g + 2], (int32_t)v[4 * g + 3]);
+                        return;
+                    }
                     const uint32_t stage = smem_epistage + (quarter * 2u + (uint32_t)(epi_chunks & 1u)) * Cfg::kEpiStageBytes;
                     if (lane == 0) ptx::bulk_wait_read<1>();       // the copy that last read this buffer (two chunks ago) is done with it
                     __syncwarp();
