@@ -32,6 +32,21 @@ __device__ __forceinline__ uint32_t mapa(uint32_t local, uint32_t rank)
     return r;
 }
 
+// one lane of the (converged) warp gets true: the issuing lane of single-thread instructions in warp-uniform code
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\telect.sync _|p, 0xFFFFFFFF;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ uint64_t pack_u64(uint32_t lo, uint32_t hi)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+    return r;
+}
+
 // ---------------------------------------------------------------- programmatic dependent launch (PDL)
 // launch_dependents: the next kernel in the stream (if launched with programmatic stream serialization) may start
 // its prologue now.  wait: block until every prerequisite grid has completed and its memory is visible.

@@ -263,46 +263,51 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             }
         }
     } else if (warp == kWarpMma) {
-        // ===================================================== a3: MMA issuer (leader CTA, one lane)
-        if (rank == 0 && lane == 0) {
+        // ===================================================== a3: MMA issuer (leader CTA; the whole warp walks the loop, one
+        // elected lane issues).  Every value the tcgen05 instructions take is warp-uniform and kept so: the ring position and
+        // phase are carried incrementally, a descriptor is the ring base's low word plus small constants (ptx::make_smem_desc
+        // layout: address >> 4 in the low bits).  Issued from a divergent single-lane branch instead, ptxas wraps every MMA in
+        // an elect / broadcast / retry loop (about 30 instructions per MMA) and the issue thread, not the tensor pipe, sets
+        // the pace: 155 clk per MMA against 128.
+        if (rank == 0) {
             constexpr uint32_t idesc = ptx::make_idesc_i8_mnmajor(256, 256);
+            constexpr uint32_t kDescPlane = Cfg::kPlaneBytes >> 4;                  // + one plane
+            constexpr uint32_t kDescK = (32u * Cfg::kRowBytes) >> 4;               // + one K-step of 32 rows
+            const bool leader_lane = ptx::elect_one();
             const uint32_t tmem_R = tmem_base;
             const uint32_t tmem_Q = tmem_base + 256;
-            uint32_t it = 0, unit = 0;
+            const uint64_t desc0 = ptx::make_smem_desc_mn_sw128(smem_planes, 1024, 1024);   // plane 0 of ring slot 0
+            const uint32_t desc_hi = (uint32_t)(desc0 >> 32);
+            uint32_t slot = 0, ph = 0, unit = 0;
             for (int sg = seg_begin; sg < seg_end; ++sg, ++unit) {
                 const Segment seg = p.segments[sg];
                 const bool off = kOffDiag && (seg.I != seg.J);
                 ptx::mbar_wait_cluster(bar_acc_empty, (unit & 1u) ^ 1u);     // epilogues of both CTAs drained TMEM
                 ptx::tc_fence_after_sync();
-                for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
-                    const uint32_t slot = it % Cfg::kPlaneStages;
-                    const uint32_t ph = (it / Cfg::kPlaneStages) & 1u;
+                for (int st = seg.stage_begin; st < seg.stage_end; ++st) {
                     ptx::mbar_wait_cluster(bar_pl_full(slot), ph);
                     ptx::tc_fence_after_sync();
-                    const uint32_t pl = smem_planes + slot * Cfg::kPlaneStageBytes;
+                    if (leader_lane) {
+                        const uint32_t lo = (uint32_t)desc0 + slot * (uint32_t)(Cfg::kPlaneStageBytes >> 4);
+                        auto desc = [&](uint32_t plane, uint32_t k) { return ptx::pack_u64(lo + plane * kDescPlane + k * kDescK, desc_hi); };
 #pragma unroll
-                    for (int k = 0; k < kStageT / 32; ++k) {
-                        const uint32_t koff = (uint32_t)k * 32u * Cfg::kRowBytes;
-                        const uint64_t d_ha = ptx::make_smem_desc_mn_sw128(pl + 0 * Cfg::kPlaneBytes + koff, 1024, 1024);
-                        const uint64_t d_la = ptx::make_smem_desc_mn_sw128(pl + 1 * Cfg::kPlaneBytes + koff, 1024, 1024);
-                        const uint32_t acc = (st != seg.stage_begin || k != 0) ? 1u : 0u;
-                        if (!off) {
-                            const uint64_t d_sa = ptx::make_smem_desc_mn_sw128(pl + 2 * Cfg::kPlaneBytes + koff, 1024, 1024);
-                            ptx::mma_i8<2>(tmem_R, d_sa, d_sa, idesc, acc);   // R (= G) = s s^T,  s = h + l
-                            ptx::mma_i8<2>(tmem_Q, d_la, d_ha, idesc, acc);   // Q (= X) = l h^T
-                        } else {
-                            const uint64_t d_hb = ptx::make_smem_desc_mn_sw128(pl + 2 * Cfg::kPlaneBytes + koff, 1024, 1024);
-                            const uint64_t d_lb = ptx::make_smem_desc_mn_sw128(pl + 3 * Cfg::kPlaneBytes + koff, 1024, 1024);
-                            const uint64_t d_nb = ptx::make_smem_desc_mn_sw128(pl + 4 * Cfg::kPlaneBytes + koff, 1024, 1024);
-                            ptx::mma_i8<2>(tmem_R, d_ha, d_hb, idesc, acc);   // R  = h_I h_J^T
-                            ptx::mma_i8<2>(tmem_R, d_la, d_lb, idesc, 1u);    // R += l_I l_J^T
-                            ptx::mma_i8<2>(tmem_Q, d_la, d_hb, idesc, acc);   // Q  = l_I h_J^T
-                            ptx::mma_i8<2>(tmem_Q, d_ha, d_nb, idesc, 1u);    // Q += h_I (-l_J)^T
+                        for (uint32_t k = 0; k < (uint32_t)kStageT / 32u; ++k) {
+                            const uint32_t acc = (st != seg.stage_begin || k != 0) ? 1u : 0u;
+                            if (!off) {
+                                ptx::mma_i8<2>(tmem_R, desc(2, k), desc(2, k), idesc, acc);   // R (= G) = s s^T,  s = h + l
+                                ptx::mma_i8<2>(tmem_Q, desc(1, k), desc(0, k), idesc, acc);   // Q (= X) = l h^T
+                            } else {
+                                ptx::mma_i8<2>(tmem_R, desc(0, k), desc(2, k), idesc, acc);   // R  = h_I h_J^T
+                                ptx::mma_i8<2>(tmem_Q, desc(1, k), desc(2, k), idesc, acc);   // Q  = l_I h_J^T
+                                ptx::mma_i8<2>(tmem_R, desc(1, k), desc(3, k), idesc, 1u);    // R += l_I l_J^T
+                                ptx::mma_i8<2>(tmem_Q, desc(0, k), desc(4, k), idesc, 1u);    // Q += h_I (-l_J)^T
+                            }
                         }
+                        ptx::mma_commit<2>(bar_pl_empty(slot), 0x3);   // planes of this stage may be overwritten (both CTAs)
                     }
-                    ptx::mma_commit<2>(bar_pl_empty(slot), 0x3);   // planes of this stage may be overwritten (both CTAs)
+                    if (++slot == (uint32_t)Cfg::kPlaneStages) { slot = 0; ph ^= 1u; }
                 }
-                ptx::mma_commit<2>(bar_acc_full, 0x3);             // accumulators complete (both CTAs)
+                if (leader_lane) ptx::mma_commit<2>(bar_acc_full, 0x3);             // accumulators complete (both CTAs)
             }
         }
     } else if (warp >= kWarpUnpack0 && warp < (uint32_t)Cfg::kWarpEpi0) {
