@@ -2,7 +2,7 @@
 // resident operands, i.e. the ceiling any kind::i8 kernel on this part can reach (SURVEY.md section 7 step 3(iii),
 // "a resident-operand tcgen05.mma.kind::i8 issue-rate microbench").
 //
-// One CTA pair per two SMs (as xengine_kernel): the leader thread issues back-to-back
+// One CTA pair per two SMs (as xengine_kernel): one elected lane of the leader's warp 0 issues back-to-back
 //     tcgen05.mma.cta_group::2.kind::i8   M = 256 (2 x 128 lanes), N = 256, K = 32, both operands MN-major SWIZZLE_128B
 // from operand tiles that sit in shared memory for the whole launch -- no TMA, no unpack, no epilogue -- alternating
 // between two TMEM accumulators.  int8 ops per MMA = 2 * 256 * 256 * 32.  bench.py reports the result as
@@ -35,7 +35,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(128, 1) int8_issue_k
     const uint32_t bar0 = base + kStages * 2 * kTileBytes;
     const uint32_t tmem_slot = bar0 + 8u * kRing;
     const uint32_t rank = ptx::cluster_ctarank();
-    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t warp = threadIdx.x >> 5;
 
     for (uint32_t w = threadIdx.x; w < kStages * 2 * kTileBytes / 4; w += blockDim.x) {
         uint32_t v = hash32(w * 2654435761u + blockIdx.x * 97u + 12345u);
@@ -58,18 +58,30 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(128, 1) int8_issue_k
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-    if (rank == 0 && warp == 0 && lane == 0) {
+    if (rank == 0 && warp == 0) {
+        // the whole warp walks the loop and one elected lane issues, with warp-uniform descriptors (ring base + constants),
+        // exactly as xengine_kernel does: issued from a divergent single-lane branch ptxas wraps every tcgen05.mma in an
+        // elect / broadcast / retry loop and the issue thread, not the tensor pipe, sets the pace
         constexpr uint32_t idesc = ptx::make_idesc_i8_mnmajor(256, 256);
+        const bool leader_lane = ptx::elect_one();
+        const uint64_t desc0 = ptx::make_smem_desc_mn_sw128(base, 1024, 1024);
+        const uint32_t desc_hi = (uint32_t)(desc0 >> 32);
         int batch = 0;
-        for (int i = 0; i < n_mma; ++i) {
-            const uint32_t st = (uint32_t)(i >> 1) % kStages;                       // one stage = 2 K-steps of 32 rows
-            const uint32_t koff = (uint32_t)(i & 1) * 32u * 128u;
-            const uint64_t da = ptx::make_smem_desc_mn_sw128(base + (2 * st) * kTileBytes + koff, 1024, 1024);
-            const uint64_t db = ptx::make_smem_desc_mn_sw128(base + (2 * st + 1) * kTileBytes + koff, 1024, 1024);
-            ptx::mma_i8<2>(tmem_base + ((i & 1) ? 256u : 0u), da, db, idesc, i >= 2 ? 1u : 0u);
-            if ((i + 1) % kBatch == 0) {
+        uint32_t st = 0;                                                             // one stage = 2 K-steps of 32 rows
+        for (int i = 0; i < n_mma; i += 2) {
+            if (leader_lane) {
+                const uint32_t lo = (uint32_t)desc0 + st * (uint32_t)((2 * kTileBytes) >> 4);
+#pragma unroll
+                for (uint32_t k = 0; k < 2; ++k) {
+                    const uint64_t da = ptx::pack_u64(lo + k * ((32u * 128u) >> 4), desc_hi);
+                    const uint64_t db = ptx::pack_u64(lo + (uint32_t)(kTileBytes >> 4) + k * ((32u * 128u) >> 4), desc_hi);
+                    ptx::mma_i8<2>(tmem_base + (k ? 256u : 0u), da, db, idesc, i >= 2 ? 1u : 0u);
+                }
+            }
+            if (++st == (uint32_t)kStages) st = 0;
+            if ((i + 2) % kBatch == 0) {
                 const int slot = batch % kRing;
-                ptx::mma_commit<2>(bar0 + 8u * slot, 0x1);
+                if (leader_lane) ptx::mma_commit<2>(bar0 + 8u * slot, 0x1);
                 ++batch;
                 if (batch >= kRing) {                                               // wait for the batch issued kRing - 1 batches ago
                     const int wb = batch - (kRing - 1) - 1;
@@ -79,7 +91,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(128, 1) int8_issue_k
         }
         // drain: one more commit behind everything issued
         const int slot = batch % kRing;
-        ptx::mma_commit<2>(bar0 + 8u * slot, 0x1);
+        if (leader_lane) ptx::mma_commit<2>(bar0 + 8u * slot, 0x1);
         for (int wb = (batch >= kRing - 1 ? batch - (kRing - 1) : 0); wb <= batch; ++wb)
             ptx::mbar_wait(bar0 + 8u * (wb % kRing), (uint32_t)(wb / kRing) & 1u);
     }
@@ -101,6 +113,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(128, 1) int8_issue_k
 extern "C" int xcorr_probe_int8_issue(int mma_per_pair, int launches, int pattern, double *tops_out, double *ms_out)
 {
     if (mma_per_pair <= 0 || launches <= 0 || pattern < 0 || pattern > 2 || !tops_out || !ms_out) return -1;
+    if (mma_per_pair % kBatch != 0) return -1;   // the issue loop commits every kBatch MMAs
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return -4;

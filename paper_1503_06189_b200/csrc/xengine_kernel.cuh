@@ -202,25 +202,31 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         ptx::mbar_init(bar_acc_empty, 2 * kNumEpiWarps);          // epilogue warps of BOTH CTAs (leader only)
         ptx::fence_mbar_init();
     }
-    if (warp == kWarpTma && lane == 0) {
-        ptx::prefetch_tensormap(&frame_map);
-        for (int s = 0; s < Cfg::kPackedStages; ++s) {
-            ptx::mbar_init(bar_pk_full(s), 1);                    // TMA producer's arrive.expect_tx
-            ptx::mbar_init(bar_pk_empty(s), Cfg::kGroupWarps);      // one arrive per unpack warp of the stage's group
+    // the TMA warp walks its loops as a whole and one elected lane issues (warp-uniform operands: see the MMA issuer)
+    bool tma_leader = false;
+    if (warp == kWarpTma) {
+        tma_leader = ptx::elect_one();
+        if (tma_leader) {
+            ptx::prefetch_tensormap(&frame_map);
+            for (int s = 0; s < Cfg::kPackedStages; ++s) {
+                ptx::mbar_init(bar_pk_full(s), 1);                    // TMA producer's arrive.expect_tx
+                ptx::mbar_init(bar_pk_empty(s), Cfg::kGroupWarps);      // one arrive per unpack warp of the stage's group
+            }
+            ptx::fence_mbar_init();
+            ptx::fence_proxy_async_smem();
         }
-        ptx::fence_mbar_init();
-        ptx::fence_proxy_async_smem();
+        __syncwarp();
         // the packed barriers and slots are this CTA's own: start the first loads now, so the frame is already on its
         // way while TMEM is allocated and the cluster synchronises
         // the frame may be the output of the previous kernel of the stream, which may have let this grid start early:
         // wait for it, unless the caller has promised complete frames (xcorr_promise_complete_frames)
         if (p.wait_frame) ptx::grid_dependency_wait();
-        // loads first (every TMA instruction costs this lane on the order of 100 clk to issue, and the first MMA waits for the
-        // first box): the L2 prefetches of the stages behind them follow after the prologue barrier
+        // loads first (the first MMA waits for the first box): the L2 prefetches of the stages behind them follow after the
+        // prologue barrier
         for (int sg = seg_begin; sg < seg_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++sg) {
             const Segment seg = p.segments[sg];
             for (int st = seg.stage_begin; st < seg.stage_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++st, ++tma_pre)
-                tma_issue(seg, st, tma_pre);
+                if (tma_leader) tma_issue(seg, st, tma_pre);
         }
     }
     if (warp == kWarpTmem) {
@@ -244,21 +250,21 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
     if (warp == kWarpTma) {
-        // ===================================================== a1: TMA producer (one lane)
-        if (lane == 0) {
+        // ===================================================== a1: TMA producer (whole warp, one elected lane issues)
+        {
             // L2 prefetch cursor: the stages loaded in the prologue need no request; then run kPrefetchStages ahead of the loads
             if (pf_sg < seg_end) { pf_seg = p.segments[pf_sg]; pf_st = pf_seg.stage_begin; }
-            for (int k = 0; k < Cfg::kPrefetchStages; ++k) prefetch_next(k >= (int)tma_pre);
-            uint32_t it = 0;
+            for (int k = 0; k < Cfg::kPrefetchStages; ++k) prefetch_next(tma_leader && k >= (int)tma_pre);
+            uint32_t it = 0, slot = 0, ph = 0;
             for (int sg = seg_begin; sg < seg_end; ++sg) {
                 const Segment seg = p.segments[sg];
                 for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
-                    prefetch_next();                               // stage it + kPrefetchStages -> L2
-                    if (it < tma_pre) continue;                    // already in flight (prologue)
-                    const uint32_t slot = it % Cfg::kPackedStages;
-                    const uint32_t ph = (it / Cfg::kPackedStages) & 1u;
-                    ptx::mbar_wait(bar_pk_empty(slot), ph ^ 1u);
-                    tma_issue(seg, st, slot);
+                    prefetch_next(tma_leader);                     // stage it + kPrefetchStages -> L2
+                    if (it >= tma_pre) {                           // (the first tma_pre stages are in flight since the prologue)
+                        ptx::mbar_wait(bar_pk_empty(slot), ph ^ 1u);
+                        if (tma_leader) tma_issue(seg, st, slot);
+                    }
+                    if (++slot == (uint32_t)Cfg::kPackedStages) { slot = 0; ph ^= 1u; }
                 }
             }
         }
