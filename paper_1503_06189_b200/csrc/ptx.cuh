@@ -123,15 +123,6 @@ __device__ __forceinline__ void tma_load_3d(uint32_t smem_dst, const CUtensorMap
         : "memory");
 }
 
-// 3-D tiled prefetch global -> L2 (no shared-memory destination, no completion to wait for): the box is on its way into L2
-// long before the load that needs it, so that load pays the L2 latency instead of the HBM latency
-__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap *m, int c0, int c1, int c2)
-{
-    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(reinterpret_cast<uint64_t>(m)), "r"(c0),
-                 "r"(c1), "r"(c2)
-                 : "memory");
-}
-
 // L2 eviction policy for data that is read exactly once (the frame): evict first, so that the accumulator slots the
 // epilogue writes stay in L2 for xcorr_read's finalize pass
 __device__ __forceinline__ uint64_t l2_policy_evict_first()

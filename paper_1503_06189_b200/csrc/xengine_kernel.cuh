@@ -1,7 +1,6 @@
 // xengine_kernel.cuh -- the fused X-engine kernel for sm_100a (hot-path rows a1..a4).
 //
-//   a1  TMA stages packed bytes  frame[t][f][128 inputs]  as 128-byte rows (SWIZZLE_128B) into smem; the same boxes are
-//       requested into L2 kPrefetchStages stages ahead (cp.async.bulk.prefetch.tensor), so the loads pay L2 latency
+//   a1  TMA stages packed bytes  frame[t][f][128 inputs]  as 128-byte rows (SWIZZLE_128B) into smem, kPackedStages deep
 //   a2  unpack warps split each byte into int8 planes (same swizzled 128-byte-row layout, so the unpack is purely
 //       element-wise and never looks at the swizzle).  The planes hold the OFFSET values h' = Re + 8, l' = Im + 8 in
 //       [0, 15] and, per tile kind, s' = h' + l' or the complement 15 - l' (layout.hpp "OFFSET OPERANDS": constant-zero
@@ -50,10 +49,6 @@ struct KernelCfg {
     static constexpr int kPackedStageBytes = kPackedBlocks * kPlaneBytes;
     static constexpr int kPlaneStageBytes = kPlanes * kPlaneBytes;
     static constexpr int kPackedStages = kOffDiag ? 4 : 8;
-    // L2 prefetch distance of the TMA lane, in stages: the box of stage it + kPrefetchStages is requested into L2 when stage
-    // `it` is loaded into shared memory.  4 packed stages in flight per SM (4.7 MB over the chip) cover only ~2.9 TB/s at
-    // the HBM latency of this access pattern (64 rows of 128 B per box); with the prefetch the loads hit L2.
-    static constexpr int kPrefetchStages = 16;
     static constexpr int kPlaneStages = kOffDiag ? 3 : 5;
     static constexpr int kUnpackWarps = 8;                         // multiple of 4
     static constexpr int kUnpackThreads = kUnpackWarps * 32;
@@ -176,21 +171,6 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         if (off)
             ptx::tma_load_3d(dst + Cfg::kPlaneBytes, &frame_map, bar_pk_full(slot), seg.J * kSuper + (int)rank * kBlock, seg.f, st * kStageT);
     };
-    // the same box requested into L2 only
-    auto tma_prefetch = [&](const Segment &seg, int st) {
-        ptx::tma_prefetch_3d(&frame_map, seg.I * kSuper + (int)rank * kBlock, seg.f, st * kStageT);
-        if (kOffDiag && (seg.I != seg.J)) ptx::tma_prefetch_3d(&frame_map, seg.J * kSuper + (int)rank * kBlock, seg.f, st * kStageT);
-    };
-    // cursor of the L2 prefetch: runs kPrefetchStages stages ahead of the loads through the worker's segment list
-    int pf_sg = seg_begin, pf_st = 0;
-    Segment pf_seg = {};
-    auto prefetch_next = [&](bool request = true) {
-        if (pf_sg >= seg_end) return;
-        if (request) tma_prefetch(pf_seg, pf_st);
-        if (++pf_st >= pf_seg.stage_end) {
-            if (++pf_sg < seg_end) { pf_seg = p.segments[pf_sg]; pf_st = pf_seg.stage_begin; }
-        }
-    };
     uint32_t tma_pre = 0;   // packed stages the TMA lane put in flight before the prologue barrier (their slots start empty)
 
     if (warp == kWarpMma && lane == 0) {
@@ -221,8 +201,6 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         // the frame may be the output of the previous kernel of the stream, which may have let this grid start early:
         // wait for it, unless the caller has promised complete frames (xcorr_promise_complete_frames)
         if (p.wait_frame) ptx::grid_dependency_wait();
-        // loads first (the first MMA waits for the first box): the L2 prefetches of the stages behind them follow after the
-        // prologue barrier
         for (int sg = seg_begin; sg < seg_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++sg) {
             const Segment seg = p.segments[sg];
             for (int st = seg.stage_begin; st < seg.stage_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++st, ++tma_pre)
@@ -252,14 +230,10 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
     if (warp == kWarpTma) {
         // ===================================================== a1: TMA producer (whole warp, one elected lane issues)
         {
-            // L2 prefetch cursor: the stages loaded in the prologue need no request; then run kPrefetchStages ahead of the loads
-            if (pf_sg < seg_end) { pf_seg = p.segments[pf_sg]; pf_st = pf_seg.stage_begin; }
-            for (int k = 0; k < Cfg::kPrefetchStages; ++k) prefetch_next(tma_leader && k >= (int)tma_pre);
             uint32_t it = 0, slot = 0, ph = 0;
             for (int sg = seg_begin; sg < seg_end; ++sg) {
                 const Segment seg = p.segments[sg];
                 for (int st = seg.stage_begin; st < seg.stage_end; ++st, ++it) {
-                    prefetch_next(tma_leader);                     // stage it + kPrefetchStages -> L2
                     if (it >= tma_pre) {                           // (the first tma_pre stages are in flight since the prologue)
                         ptx::mbar_wait(bar_pk_empty(slot), ph ^ 1u);
                         if (tma_leader) tma_issue(seg, st, slot);
