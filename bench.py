@@ -331,6 +331,9 @@ def tensor_roofline(cfg, k_ms, peaks, ceiling=None):
     return r
 
 
+C3_POOL = 4     # distinct seeded frames the 64-frame streamed run cycles through (1 GiB each, page-locked)
+
+
 def measure_other_config(name, xb, torch, peaks, ceiling, steps=20):
     """C4 / C5 (device-resident step) and C3 (device-resident step + the 64-frame streamed run of BASELINE.json configs[2])."""
     cfg = wl.CONFIGS[name]
@@ -362,16 +365,19 @@ def measure_other_config(name, xb, torch, peaks, ceiling, steps=20):
         out["added_frame_kernel_ms"] = e0.elapsed_time(e1) / steps
         # BASELINE.json configs[2]: n_frames consecutive frames from pinned host memory, double-buffered H2D overlapped with
         # the correlation, ONE read at the end
-        pinned = [torch.from_numpy(f).pin_memory() for f in r.host_frames]
+        # (BASELINE.json configs[2]: 64 consecutive seeded frames; a pool of C3_POOL distinct seeded frames is cycled, as
+        # SURVEY.md section 8(d) allows -- the same pool size tests/test_gpu_parity.py::test_c3_streamed_64_frames checks)
+        pool = r.host_frames + [cfg.frame(k) for k in range(len(r.host_frames), C3_POOL)]
+        pinned = [torch.from_numpy(f).pin_memory() for f in pool]
         out_host = torch.empty((cfg.n_freq, cfg.n_pairs, 2), dtype=torch.int32).pin_memory()
         s = xb.XCorrStream(r.x, depth=2)
         for k in range(2):
-            s.submit(pinned[k % 2])
+            s.submit(pinned[k % C3_POOL])
         s.read(out_host)
         barrier()
         t0 = time.perf_counter()
         for k in range(cfg.n_frames):
-            s.submit(pinned[k % 2])
+            s.submit(pinned[k % C3_POOL])
         s.read(out_host)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
@@ -379,15 +385,15 @@ def measure_other_config(name, xb, torch, peaks, ceiling, steps=20):
         torch.cuda.synchronize()
         t1 = time.perf_counter()
         for k in range(4):
-            hb.copy_(pinned[k % 2].view(-1), non_blocking=True)
+            hb.copy_(pinned[k % C3_POOL].view(-1), non_blocking=True)
         torch.cuda.synchronize()
         h2d = 8.0 * 4 * cfg.frame_bytes / (time.perf_counter() - t1) / 1e9
         del hb
         s.close()
         out["streamed"] = {"value": 8.0 * cfg.frame_bytes * cfg.n_frames / dt / 1e9, "unit": "Gb/s", "frames": cfg.n_frames,
-                           "pool": 2, "ms_per_frame": dt / cfg.n_frames * 1e3, "h2d_only_gbps": h2d, "paper_rate_gbps": 819.2,
+                           "pool": C3_POOL, "ms_per_frame": dt / cfg.n_frames * 1e3, "h2d_only_gbps": h2d, "paper_rate_gbps": 819.2,
                            "h2d_bytes_per_frame": cfg.frame_bytes, "d2h_bytes_total": cfg.output_bytes,
-                           "api": f"{cfg.n_frames} x xcorr_stream_submit(pinned host frame, pool of 2 distinct frames cycled) + one "
+                           "api": f"{cfg.n_frames} x xcorr_stream_submit(pinned host frame, pool of {C3_POOL} distinct frames cycled) + one "
                                   "xcorr_stream_read(pinned host out); host wall clock from the first submit to the result in host memory"}
     r.close()
     torch.cuda.empty_cache()

@@ -34,6 +34,7 @@ struct xcorr_handle {
     int n_workers = 0;
     int n_sms = 0;
     int n_tiles = 0;                 // F * n_supertiles
+    Segment head[kMaxHeadWorkers];   // first segment of every worker, copied into KernelParams at each launch
     bool offdiag = false;            // N > 256: kernel variant with the column block and -Im plane
     size_t frame_bytes = 0, output_bytes = 0, acc_bytes = 0;
     int32_t *acc = nullptr;          // device accumulator slots (layout.hpp), one per work segment
@@ -223,6 +224,10 @@ extern "C" int xcorr_create(int n_inputs, int n_freq, int t_per_frame, xcorr_han
     Schedule sched;
     if ((rc = make_schedule_noexcept(n_inputs, n_freq, t_per_frame, h->n_workers, &sched)) != XCORR_OK) return fail(rc);
     if (cudaEventCreateWithFlags(&h->order_event, cudaEventDisableTiming) != cudaSuccess) return fail(XCORR_ECUDA);
+    for (int w = 0; w < kMaxHeadWorkers; ++w) {   // KernelParams::head: the first segment of every worker
+        h->head[w] = Segment{};
+        if (w < h->n_workers && sched.worker_begin[w] < sched.worker_begin[w + 1]) h->head[w] = sched.segments[sched.worker_begin[w]];
+    }
     h->n_slots = (int)sched.segments.size();
     h->acc_bytes = (size_t)h->n_slots * kAccElemsPerSlot * sizeof(int32_t);
     cudaError_t e;
@@ -292,6 +297,7 @@ extern "C" int xcorr_process(xcorr_handle *h, const void *packed_frame_dev, void
     if (rc != XCORR_OK) return rc;
     if ((rc = order_after_previous(h, (cudaStream_t)cuda_stream)) != XCORR_OK) return rc;
     KernelParams p;
+    for (int w = 0; w < kMaxHeadWorkers; ++w) p.head[w] = h->head[w];
     p.segments = h->segments;
     p.worker_begin = h->worker_begin;
     p.acc = h->acc;

@@ -97,7 +97,13 @@ constexpr int kWarpTmem = 2;
 constexpr int kWarpUnpack0 = 4;        // unpack warps 4 .. 4 + Cfg::kUnpackWarps - 1, then 4 epilogue warps
 constexpr int kNumEpiWarps = 4;
 
+constexpr int kMaxHeadWorkers = 80;   // workers whose first segment also travels in the kernel parameters (74 on a B200)
+
 struct KernelParams {
+    // every worker's FIRST segment, in the parameter (constant) bank: the schedule tables below are evicted from L2 by every
+    // frame that streams through, and two dependent cold loads (worker_begin -> segments) kept the first frame load back by
+    // about 2 k clk.  A worker without segments has stage_begin == stage_end here.
+    Segment head[kMaxHeadWorkers];
     const Segment *segments;       // device
     const int32_t *worker_begin;   // device, n_workers + 1
     int32_t *acc;                  // device accumulator slots, layout.hpp
@@ -201,8 +207,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
         // the frame may be the output of the previous kernel of the stream, which may have let this grid start early:
         // wait for it, unless the caller has promised complete frames (xcorr_promise_complete_frames)
         if (p.wait_frame) ptx::grid_dependency_wait();
-        for (int sg = seg_begin; sg < seg_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++sg) {
-            const Segment seg = p.segments[sg];
+        // (the first segment's stages only: its description comes with the kernel parameters, see KernelParams::head)
+        if (worker < (uint32_t)kMaxHeadWorkers) {
+            const Segment seg = p.head[worker];
             for (int st = seg.stage_begin; st < seg.stage_end && tma_pre < (uint32_t)Cfg::kPackedStages; ++st, ++tma_pre)
                 if (tma_leader) tma_issue(seg, st, tma_pre);
         }
