@@ -1,11 +1,13 @@
 // schedule.hpp -- host-side work decomposition for the persistent X-engine kernel (pure C++, no CUDA).
 //
 // Work item  = one super-tile (f, I <= J) over the whole frame; it is cut along time into STAGES of
-//              kStageT samples.  Cost model per stage: 11 for a diagonal item (I == J), 16 for an off-diagonal one --
-//              measured, not counted: a diagonal K-step is 2 MMAs against 4, but in the N > 256 kernel
-//              both forms are bound by the shared-memory side and the diagonal one keeps less of its advantage.  Sweep of
-//              the diagonal cost at 16 for the other (C4 / C5 xcorr_process, us): 9: 656 / 1413, 10: 646 / 1354,
-//              11: 645 / 1355, 12: 654 / 1447, 13: 658 / 1518.  N <= 256 has diagonal items only, any constant does.
+//              kStageT samples.  Cost model per stage: 16 for an off-diagonal item (2 x 4 MMAs of 128 clk: the kernel runs at
+//              the tensor pipe's floor) and 9 for a diagonal one (2 x 2 MMAs would be 8; in the N > 256
+//              kernel, whose rings are sized for the off-diagonal form, the diagonal stages run a little above their
+//              floor).  Measured, not only counted -- xcorr_process (us) at C4 / C5 by diagonal cost: 8: 558 / 1266,
+//              9: 547 / 1201, 10: 551 / 1218, 11 (the model of the earlier, issue-bound kernel): 561 / 1280.  N <= 256 has
+//              diagonal items only, any constant does.  (A per-segment cost for the accumulator drain, during which the
+//              worker's tensor pipe idles, was tried on top: no measurable gain at C2..C5, left out.)
 // Worker     = one CTA pair (two SMs, one 2-CTA tcgen05 MMA stream); there are `n_workers` of them.
 //
 // Hybrid data-parallel / stream-K split (integer addition is exact and order independent, so a
@@ -58,7 +60,7 @@ inline Schedule make_schedule(int n_inputs, int n_freq, int n_time, int n_worker
     for (int f = 0; f < n_freq; ++f)
         for (int I = 0; I < nb; ++I)
             for (int J = I; J < nb; ++J)
-                items.push_back({f, I, J, f * nst + (I * (2 * nb - I + 1) / 2 + (J - I)), I == J ? 11 : 16});
+                items.push_back({f, I, J, f * nst + (I * (2 * nb - I + 1) / 2 + (J - I)), I == J ? 9 : 16});
 
     const int64_t n_items = (int64_t)items.size();
     // whole rounds of n_workers items go data-parallel only as long as no worker ends above the mean load of the whole job
