@@ -12,7 +12,8 @@
 //   acc[slot][r][row / 32][col / 4][row % 32][col % 4]   int32,   r in {0,1}, col in [0,512), row in [0,128)
 //
 // i.e. per epilogue warp (32 TMEM lanes) the columns run contiguously: a chunk of 32 columns is one 4 KiB piece, which
-// the epilogue stages in shared memory and hands to ONE bulk copy (first frame) or bulk int32 reduce-add (later frames).
+// the epilogue writes with eight 16-byte stores per lane (first frame: 512 contiguous bytes per warp and instruction) or
+// stages in shared memory and hands to ONE bulk int32 reduce-add (later frames).
 //
 //     row          = TMEM lane       : input  i = 256*I + 128*r + row
 //     col in [0,256)  "R" columns    : input  j = 256*J + col
