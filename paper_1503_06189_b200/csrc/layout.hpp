@@ -47,6 +47,7 @@ namespace xc {
 constexpr int kBlock = 128;        // inputs per CTA row block (TMEM lanes)
 constexpr int kSuper = 256;        // inputs per super-block (CTA pair)
 constexpr int kAccCols = 512;      // TMEM columns per CTA: 256 R + 256 Q
+constexpr int kDiagSplitCol = 192; // diagonal super-tiles: G[i < 128, j >= 192] is written by CTA half 1 (from its transposed copy) into half 0's place
 constexpr int kAccElemsPerCta = kAccCols * kBlock;          // 65536 int32
 constexpr int kAccElemsPerQuarter = kAccCols * 32;          // 16384 int32: the 32 TMEM lanes one epilogue warp owns
 constexpr int kAccElemsPerSlot = 2 * kAccElemsPerCta;        // 131072 int32 = 512 KiB

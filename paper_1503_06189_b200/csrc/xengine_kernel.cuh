@@ -484,11 +484,22 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 released = true;
             };
             if (rows_valid > 0) {
-                // R columns: on a diagonal super-tile only j >= i is ever read -> start at this warp's first row
-                const int r_begin = (seg.I == seg.J) ? row0 : 0;
-                const int n_chunks_r = max((cols_valid - r_begin + 31) / 32, 0);
+                // R columns.  On a diagonal super-tile R (= G) is symmetric and only j >= i is wanted: a warp starts at its first
+                // row, and the 128 x 128 block G[0:128, 128:256] -- held by CTA 0 as is and by CTA 1 transposed -- is SHARED between
+                // the two CTAs: CTA 0 writes its columns 128..191, CTA 1 writes the rest from its rows 192..255, columns 0..127,
+                // turned around on the way through the staging buffer and put where CTA 0 would have put it (the slot layout does
+                // not change).  Both CTAs then drain 50 chunks instead of 58 and 42, and the drain -- bound by each SM's 30 B/clk
+                // store path while the tensor pipe waits -- is as long as its longer half.
+                const bool diag = (seg.I == seg.J);
+                const int ra_begin = diag ? row0 : 0;
+                const int ra_end = (diag && rank == 0) ? min(cols_valid, kDiagSplitCol) : cols_valid;
+                const int rb_end = (diag && rank == 1 && row0 >= kDiagSplitCol) ? min(cols_valid, kBlock) : 0;   // columns [0, rb_end)
+                const int n_chunks_a = max((ra_end - ra_begin + 31) / 32, 0);
+                const int n_chunks_r = n_chunks_a + (rb_end + 31) / 32;
                 const int n_chunks = n_chunks_r + (cols_valid + 31) / 32;       // R chunks, then Q chunks (32 columns each)
-                auto chunk_col = [&](int ch) { return (ch < n_chunks_r) ? (r_begin + 32 * ch) : (256 + 32 * (ch - n_chunks_r)); };
+                auto chunk_col = [&](int ch) {
+                    return (ch < n_chunks_a) ? (ra_begin + 32 * ch) : (ch < n_chunks_r) ? 32 * (ch - n_chunks_a) : (256 + 32 * (ch - n_chunks_r));
+                };
                 auto chunk_load = [&](int ch, uint32_t (&v)[32]) {
                     ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + (uint32_t)chunk_col(ch), v);
                 };
@@ -496,8 +507,10 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 // handed to ONE bulk copy (first frame of an integration) or bulk int32 reduce-add (later frames: the addition
                 // happens at the destination, nothing is loaded into the SM).  Two staging buffers per warp; lane 0 owns the
                 // bulk groups.
+                int32_t *slot_peer_cols = p.acc + ((size_t)seg.slot * 2 + 0) * (size_t)kAccElemsPerCta + (size_t)(row0 >> 2) * (32 * 4);
                 auto chunk_store = [&](int ch, const uint32_t (&v)[32]) {
-                    if (p.first_frame) {
+                    const bool turned = ch >= n_chunks_a && ch < n_chunks_r;      // CTA 1's share of G[0:128, 128:256], see above
+                    if (p.first_frame && !turned) {
                         // first frame of an integration: plain stores straight from the registers -- lane = row, 16 bytes per
                         // lane and instruction = 512 contiguous bytes of the slot per warp; no staging, no proxy fence, no bulk
                         // group (an epilogue of 16 chunks: 8.5 k -> about 4 k clk, which is what reading TMEM costs)
@@ -510,15 +523,24 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                     const uint32_t stage = smem_epistage + (quarter * 2u + (uint32_t)(epi_chunks & 1u)) * Cfg::kEpiStageBytes;
                     if (lane == 0) ptx::bulk_wait_read<1>();       // the copy that last read this buffer (two chunks ago) is done with it
                     __syncwarp();
+                    if (!turned) {
 #pragma unroll
-                    for (int g = 0; g < 8; ++g)
-                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(stage + (uint32_t)g * 512u + lane * 16u), "r"(v[4 * g]),
-                                     "r"(v[4 * g + 1]), "r"(v[4 * g + 2]), "r"(v[4 * g + 3])
-                                     : "memory");
+                        for (int g = 0; g < 8; ++g)
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(stage + (uint32_t)g * 512u + lane * 16u), "r"(v[4 * g]),
+                                         "r"(v[4 * g + 1]), "r"(v[4 * g + 2]), "r"(v[4 * g + 3])
+                                         : "memory");
+                    } else {
+                        // this lane's row j = row0 + lane becomes COLUMN lane of the chunk, its column k becomes row k:
+                        // the chunk [col / 4][row][col % 4] of rows 32 c .. 32 c + 31 (c = chunk_col / 32) of CTA half 0
+#pragma unroll
+                        for (int k = 0; k < 32; ++k)
+                            asm volatile("st.shared.u32 [%0], %1;" ::"r"(stage + (lane >> 2) * 512u + (lane & 3u) * 4u + (uint32_t)k * 16u), "r"(v[k]) : "memory");
+                    }
                     ptx::fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) {
-                        int32_t *dst = slot_warp + (size_t)(chunk_col(ch) >> 2) * (32 * 4);
+                        int32_t *dst = turned ? slot_peer_cols + (size_t)(chunk_col(ch) >> 5) * (size_t)kAccElemsPerQuarter
+                                              : slot_warp + (size_t)(chunk_col(ch) >> 2) * (32 * 4);
                         if (p.first_frame) ptx::bulk_store(dst, stage, Cfg::kEpiStageBytes);
                         else ptx::bulk_reduce_add_s32(dst, stage, Cfg::kEpiStageBytes);
                         ptx::bulk_commit();
