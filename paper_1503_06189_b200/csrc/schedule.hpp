@@ -83,12 +83,13 @@ inline Schedule make_schedule(int n_inputs, int n_freq, int n_time, int n_worker
         }
     }
     std::vector<std::vector<Segment>> per(n_workers);
+    std::vector<std::vector<Segment>> per_dp(n_workers);   // the whole items of the data-parallel rounds
     std::vector<int64_t> load(n_workers, 0);
 
     for (int64_t u = 0; u < n_dp; ++u) {
         const Item &it = items[u];
         const int w = (int)(u % n_workers);
-        per[w].push_back({it.f, it.I, it.J, 0, s.n_stages, it.tile, 0, 0});
+        per_dp[w].push_back({it.f, it.I, it.J, 0, s.n_stages, it.tile, 0, 0});
         load[w] += it.cost_per_stage * s.n_stages;
     }
 
@@ -133,6 +134,17 @@ inline Schedule make_schedule(int n_inputs, int n_freq, int n_time, int n_worker
                 st += take;
             }
         }
+    }
+
+    // Order inside a worker.  N > 256: the data-parallel rounds first -- all workers start them together, so neighbouring
+    // super-tiles of a channel walk through time side by side and share their blocks through L2.  N <= 256 (nothing to
+    // share): the worker's FIRST water-filled piece, then its whole items, then the rest -- that piece is the tail of an
+    // item and its length differs from worker to worker (the cut points of the water filling fall anywhere), so all later
+    // item boundaries, where an SM drains its accumulators at 30 B/clk, are spread over the item period instead of hitting
+    // L2 from all 148 SMs at once.
+    for (int w = 0; w < n_workers; ++w) {
+        const size_t at = (nb > 1 || per[w].empty()) ? 0 : 1;
+        per[w].insert(per[w].begin() + at, per_dp[w].begin(), per_dp[w].end());
     }
 
     // slots: one per segment, numbered in (tile, stage_begin) order so that a tile's slots are contiguous
