@@ -510,7 +510,34 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 int32_t *slot_peer_cols = p.acc + ((size_t)seg.slot * 2 + 0) * (size_t)kAccElemsPerCta + (size_t)(row0 >> 2) * (32 * 4);
                 auto chunk_store = [&](int ch, const uint32_t (&v)[32]) {
                     const bool turned = ch >= n_chunks_a && ch < n_chunks_r;      // CTA 1's share of G[0:128, 128:256], see above
-                    if (p.first_frame && !turned) {
+                    if (p.first_frame && turned) {
+                        // turned around in registers: the four lanes of a quad (rows j = 4 g .. 4 g + 3 of this warp) exchange
+                        // 4 x 4 blocks, after which lane (g, m) holds, for rows i = 4 t + m of the chunk, the four columns
+                        // 4 g .. 4 g + 3 -- 16 bytes of CTA 0's slot each, 64 contiguous bytes per quad.  Register indices stay
+                        // static: a lane rotates its block row by m before sending and the received column by m afterwards.
+                        const uint32_t m = lane & 3u, quad = lane & ~3u;
+                        int32_t *dst = slot_peer_cols + (size_t)(chunk_col(ch) >> 5) * (size_t)kAccElemsPerQuarter + (lane >> 2) * (32 * 4) + m * 4;
+                        auto rot4 = [&](uint32_t (&a)[4], uint32_t by) {         // a[c] <- a[(c + by) & 3]
+                            if (by & 1u) { const uint32_t t0 = a[0]; a[0] = a[1]; a[1] = a[2]; a[2] = a[3]; a[3] = t0; }
+                            if (by & 2u) { const uint32_t t0 = a[0], t1 = a[1]; a[0] = a[2]; a[1] = a[3]; a[2] = t0; a[3] = t1; }
+                        };
+#pragma unroll
+                        for (int t = 0; t < 8; ++t) {
+                            uint32_t u[4] = {v[4 * t], v[4 * t + 1], v[4 * t + 2], v[4 * t + 3]};
+                            rot4(u, m);                                           // u[r] = this row's column 4 t + ((m + r) & 3)
+                            uint32_t o[4];
+                            o[0] = u[0];                                          // own row, column 4 t + m
+#pragma unroll
+                            for (int r = 1; r < 4; ++r)                           // from lane (m - r) & 3: its row, column 4 t + m
+                                o[r] = __shfl_sync(0xFFFFFFFFu, u[r], (int)(quad + ((m - (uint32_t)r) & 3u)));
+                            // o[r] belongs to source row (m - r) & 3: put the rows in order 0..3
+                            uint32_t w[4] = {o[0], o[3], o[2], o[1]};             // w[c] = row (m + c) & 3
+                            rot4(w, (4u - m) & 3u);                               // w[c] <- row c
+                            ptx::st_global_v4(dst + t * 16, (int32_t)w[0], (int32_t)w[1], (int32_t)w[2], (int32_t)w[3]);
+                        }
+                        return;
+                    }
+                    if (p.first_frame) {
                         // first frame of an integration: plain stores straight from the registers -- lane = row, 16 bytes per
                         // lane and instruction = 512 contiguous bytes of the slot per warp; no staging, no proxy fence, no bulk
                         // group (an epilogue of 16 chunks: 8.5 k -> about 4 k clk, which is what reading TMEM costs)
