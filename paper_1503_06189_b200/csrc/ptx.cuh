@@ -226,12 +226,8 @@ __device__ __forceinline__ int4 ld_global_v4(const int32_t *addr)
     return r;
 }
 
-// ---------------------------------------------------------------- bulk (TMA) stores smem -> global, issued by one thread
-__device__ __forceinline__ void bulk_store(void *gdst, uint32_t smem_src, uint32_t bytes)
-{
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_src), "r"(bytes) : "memory");
-}
-// the same as an int32 add performed at the destination (no load in the SM: the reduction happens in L2)
+// ---------------------------------------------------------------- bulk (TMA) reduce smem -> global, issued by one thread
+// int32 add performed at the destination (no load in the SM: the reduction happens in L2)
 __device__ __forceinline__ void bulk_reduce_add_s32(void *gdst, uint32_t smem_src, uint32_t bytes)
 {
     asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.s32 [%0], [%1], %2;" ::"l"(gdst), "r"(smem_src), "r"(bytes)

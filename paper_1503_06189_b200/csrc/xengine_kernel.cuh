@@ -503,20 +503,15 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 auto chunk_load = [&](int ch, uint32_t (&v)[32]) {
                     ptx::tmem_ld_32x32(tmem_base + ((quarter * 32u) << 16) + (uint32_t)chunk_col(ch), v);
                 };
-                // a chunk leaves through shared memory: 32 lanes x 8 x 16 bytes = the 4 KiB piece of the slot in its final order,
-                // handed to ONE bulk copy (first frame of an integration) or bulk int32 reduce-add (later frames: the addition
-                // happens at the destination, nothing is loaded into the SM).  Two staging buffers per warp; lane 0 owns the
-                // bulk groups.
                 int32_t *slot_peer_cols = p.acc + ((size_t)seg.slot * 2 + 0) * (size_t)kAccElemsPerCta + (size_t)(row0 >> 2) * (32 * 4);
-                auto chunk_store = [&](int ch, const uint32_t (&v)[32]) {
+                auto chunk_store = [&](int ch, uint32_t (&v)[32]) {
                     const bool turned = ch >= n_chunks_a && ch < n_chunks_r;      // CTA 1's share of G[0:128, 128:256], see above
-                    if (p.first_frame && turned) {
+                    const uint32_t m = lane & 3u, quad = lane & ~3u;
+                    if (turned) {
                         // turned around in registers: the four lanes of a quad (rows j = 4 g .. 4 g + 3 of this warp) exchange
-                        // 4 x 4 blocks, after which lane (g, m) holds, for rows i = 4 t + m of the chunk, the four columns
-                        // 4 g .. 4 g + 3 -- 16 bytes of CTA 0's slot each, 64 contiguous bytes per quad.  Register indices stay
-                        // static: a lane rotates its block row by m before sending and the received column by m afterwards.
-                        const uint32_t m = lane & 3u, quad = lane & ~3u;
-                        int32_t *dst = slot_peer_cols + (size_t)(chunk_col(ch) >> 5) * (size_t)kAccElemsPerQuarter + (lane >> 2) * (32 * 4) + m * 4;
+                        // 4 x 4 blocks, after which lane (g, m) holds in v[4 t .. 4 t + 3], for row i = 4 t + m of the chunk, the
+                        // four columns 4 g .. 4 g + 3 -- 16 bytes of CTA 0's slot each, 64 contiguous bytes per quad.  Register
+                        // indices stay static: a lane rotates its block row by m before sending, the received column by -m after.
                         auto rot4 = [&](uint32_t (&a)[4], uint32_t by) {         // a[c] <- a[(c + by) & 3]
                             if (by & 1u) { const uint32_t t0 = a[0]; a[0] = a[1]; a[1] = a[2]; a[2] = a[3]; a[3] = t0; }
                             if (by & 2u) { const uint32_t t0 = a[0], t1 = a[1]; a[0] = a[2]; a[1] = a[3]; a[2] = t0; a[3] = t1; }
@@ -530,46 +525,42 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
 #pragma unroll
                             for (int r = 1; r < 4; ++r)                           // from lane (m - r) & 3: its row, column 4 t + m
                                 o[r] = __shfl_sync(0xFFFFFFFFu, u[r], (int)(quad + ((m - (uint32_t)r) & 3u)));
-                            // o[r] belongs to source row (m - r) & 3: put the rows in order 0..3
-                            uint32_t w[4] = {o[0], o[3], o[2], o[1]};             // w[c] = row (m + c) & 3
+                            uint32_t w[4] = {o[0], o[3], o[2], o[1]};             // o[r] is source row (m - r) & 3;  w[c] = row (m + c) & 3
                             rot4(w, (4u - m) & 3u);                               // w[c] <- row c
-                            ptx::st_global_v4(dst + t * 16, (int32_t)w[0], (int32_t)w[1], (int32_t)w[2], (int32_t)w[3]);
+                            v[4 * t] = w[0]; v[4 * t + 1] = w[1]; v[4 * t + 2] = w[2]; v[4 * t + 3] = w[3];
                         }
-                        return;
                     }
+                    // where vector g (v[4 g .. 4 g + 3]) of this lane goes inside the 4 KiB chunk [col / 4][row][col % 4]:
+                    // as loaded, lane = row and g = column group; turned, (lane / 4) = column group and 4 g + m = row
+                    const uint32_t vec0 = turned ? (lane >> 2) * 512u + m * 16u : lane * 16u;      // bytes
+                    const uint32_t vec_step = turned ? 64u : 512u;
+                    int32_t *chunk = turned ? slot_peer_cols + (size_t)(chunk_col(ch) >> 5) * (size_t)kAccElemsPerQuarter
+                                            : slot_warp + (size_t)(chunk_col(ch) >> 2) * (32 * 4);
                     if (p.first_frame) {
-                        // first frame of an integration: plain stores straight from the registers -- lane = row, 16 bytes per
-                        // lane and instruction = 512 contiguous bytes of the slot per warp; no staging, no proxy fence, no bulk
-                        // group (an epilogue of 16 chunks: 8.5 k -> about 4 k clk, which is what reading TMEM costs)
-                        int32_t *dst = slot_warp + (size_t)(chunk_col(ch) >> 2) * (32 * 4) + lane * 4;
+                        // first frame of an integration: plain stores straight from the registers -- 16 bytes per lane and
+                        // instruction, 512 (turned: 8 x 64) contiguous bytes of the slot per warp; no staging, no proxy fence, no
+                        // bulk group
+                        int32_t *dst = chunk + (vec0 >> 2);
 #pragma unroll
                         for (int g = 0; g < 8; ++g)
-                            ptx::st_global_v4(dst + g * (32 * 4), (int32_t)v[4 * g], (int32_t)v[4 * g + 1], (int32_t)v[4 * g + 2], (int32_t)v[4 * g + 3]);
+                            ptx::st_global_v4(dst + g * (int)(vec_step >> 2), (int32_t)v[4 * g], (int32_t)v[4 * g + 1], (int32_t)v[4 * g + 2], (int32_t)v[4 * g + 3]);
                         return;
                     }
+                    // later frames: the chunk is staged in shared memory in its final order and handed to ONE bulk int32 reduce-add
+                    // (the addition happens at the destination, nothing is loaded into the SM).  Two staging buffers per warp;
+                    // lane 0 owns the bulk groups.
                     const uint32_t stage = smem_epistage + (quarter * 2u + (uint32_t)(epi_chunks & 1u)) * Cfg::kEpiStageBytes;
                     if (lane == 0) ptx::bulk_wait_read<1>();       // the copy that last read this buffer (two chunks ago) is done with it
                     __syncwarp();
-                    if (!turned) {
 #pragma unroll
-                        for (int g = 0; g < 8; ++g)
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(stage + (uint32_t)g * 512u + lane * 16u), "r"(v[4 * g]),
-                                         "r"(v[4 * g + 1]), "r"(v[4 * g + 2]), "r"(v[4 * g + 3])
-                                         : "memory");
-                    } else {
-                        // this lane's row j = row0 + lane becomes COLUMN lane of the chunk, its column k becomes row k:
-                        // the chunk [col / 4][row][col % 4] of rows 32 c .. 32 c + 31 (c = chunk_col / 32) of CTA half 0
-#pragma unroll
-                        for (int k = 0; k < 32; ++k)
-                            asm volatile("st.shared.u32 [%0], %1;" ::"r"(stage + (lane >> 2) * 512u + (lane & 3u) * 4u + (uint32_t)k * 16u), "r"(v[k]) : "memory");
-                    }
+                    for (int g = 0; g < 8; ++g)
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(stage + vec0 + (uint32_t)g * vec_step), "r"(v[4 * g]),
+                                     "r"(v[4 * g + 1]), "r"(v[4 * g + 2]), "r"(v[4 * g + 3])
+                                     : "memory");
                     ptx::fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) {
-                        int32_t *dst = turned ? slot_peer_cols + (size_t)(chunk_col(ch) >> 5) * (size_t)kAccElemsPerQuarter
-                                              : slot_warp + (size_t)(chunk_col(ch) >> 2) * (32 * 4);
-                        if (p.first_frame) ptx::bulk_store(dst, stage, Cfg::kEpiStageBytes);
-                        else ptx::bulk_reduce_add_s32(dst, stage, Cfg::kEpiStageBytes);
+                        ptx::bulk_reduce_add_s32(chunk, stage, Cfg::kEpiStageBytes);
                         ptx::bulk_commit();
                     }
                     ++epi_chunks;
