@@ -7,14 +7,14 @@
 //       upper bits cut the MMA datapath's switching power, and the part is power-limited); the same warps keep per-input
 //       column sums of h', l' so that xcorr_read can remove the offsets exactly.  The 8 unpack warps work in groups on
 //       alternate stages (KernelCfg::kUnpackGroups)
-//   a3  one thread issues 2-CTA tcgen05.mma kind::i8 (M = 256 over the CTA pair, N = 256, K = 32) with
-//       both operands MN-major straight from those planes; int32 accumulators stay in TMEM (512 columns)
-//       for the whole time range of the work segment
-//   a4  epilogue warps tcgen05.ld the accumulators, stage them in shared memory and bulk-copy (first frame) or bulk
-//       reduce-add (later frames) them into this segment's accumulator slot
+//   a3  one elected lane of the MMA warp issues 2-CTA tcgen05.mma kind::i8 (M = 256 over the CTA pair, N = 256, K = 32)
+//       with both operands MN-major straight from those planes, every operand warp-uniform; int32 accumulators stay in
+//       TMEM (512 columns) for the whole time range of the work segment
+//   a4  epilogue warps tcgen05.ld the accumulators and write them into this segment's accumulator slot: 16-byte stores
+//       (first frame of an integration) or, through a shared-memory staging buffer, bulk reduce-adds (later frames)
 //
 // Complex product from real GEMMs (BASELINE.json:north_star (b)); h = Re plane, l = Im plane, s = h + l (offset values):
-//   off-diagonal        (I <  J):   R += h_I h_J^T ; R += l_I l_J^T ; Q += l_I h_J^T ; Q += h_I (15 - l_J)^T     (4 MMAs per K-step)
+//   off-diagonal        (I <  J):   R += h_I h_J^T ; Q += l_I h_J^T ; R += l_I l_J^T ; Q += h_I (15 - l_J)^T     (4 MMAs per K-step)
 //   diagonal super-tile (I == J):   R += s s^T ; Q += l h^T                                                     (2 MMAs per K-step)
 // On the diagonal the tile is Hermitian, which lets three real products per complex MAC do (Gauss), two of them being the
 // two triangles of ONE full product:  with G = (h+l)(h+l)^T = hh^T + ll^T + hl^T + lh^T (symmetric) and X = l h^T,
