@@ -41,8 +41,8 @@ import workloads as wl  # noqa: E402
 NOMINAL_INT8_TOPS = 4500.0  # dense int8, B200 nominal (2x the 2.25 PFLOP/s dense bf16 figure)
 # dram__bytes_read.sum + dram__bytes_write.sum of xengine_kernel<false> for one C2 launch, from the committed
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-# profiles/r02_ncu_full_bench_c2.md (268.5 MB read + 8.8 MB written) and r02_ncu_full_bench_c4_c5.md
-NCU_TRAFFIC_BYTES = {"C2": 277.28e6, "C3": None, "C4": 663.8e6, "C5": 4163.0e6}
+# profiles/r02_ncu_full_bench_c2.md (268.5 MB read + 9.6 MB written) and r02_ncu_full_bench_c4_c5.md
+NCU_TRAFFIC_BYTES = {"C2": 278.08e6, "C3": None, "C4": 675.4e6, "C5": 4156.4e6}
 # tcgen05 MMAs (M256 N256 K32, 2 CTAs) xengine_kernel issues per 32-sample K-step of a 256 x 256 super-tile
 MMAS_DIAG, MMAS_OFFDIAG = 2, 4
 
