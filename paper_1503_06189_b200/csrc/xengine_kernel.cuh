@@ -472,8 +472,8 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
             const int row0 = (int)(rank * kBlock + quarter * 32);             // first row of this warp inside the super-block
             const int rows_valid = p.n_inputs - seg.I * kSuper - row0;         // rows of this warp that are real inputs
             const int cols_valid = min(kSuper, p.n_inputs - seg.J * kSuper);   // columns that are real inputs
-            // this segment's own slot: [r][col/4][row][4] int32 -> one warp's 16-byte accesses are 512 B contiguous
-            // this warp's 64 KiB of the segment's own slot: [col / 4][row % 32][4] int32, columns contiguous
+            // this warp's 64 KiB of the segment's own slot: [col / 4][row % 32][4] int32, columns contiguous -> one warp's 16-byte
+            // accesses are 512 B contiguous
             int32_t *slot_warp = p.acc + ((size_t)seg.slot * 2 + rank) * (size_t)kAccElemsPerCta + (size_t)quarter * kAccElemsPerQuarter;
             // this warp's last TMEM load has landed: the next unit's MMAs may overwrite the accumulators
             bool released = false;
@@ -487,9 +487,9 @@ xengine_kernel(const __grid_constant__ CUtensorMap frame_map, const KernelParams
                 // R columns.  On a diagonal super-tile R (= G) is symmetric and only j >= i is wanted: a warp starts at its first
                 // row, and the 128 x 128 block G[0:128, 128:256] -- held by CTA 0 as is and by CTA 1 transposed -- is SHARED between
                 // the two CTAs: CTA 0 writes its columns 128..191, CTA 1 writes the rest from its rows 192..255, columns 0..127,
-                // turned around on the way through the staging buffer and put where CTA 0 would have put it (the slot layout does
-                // not change).  Both CTAs then drain 50 chunks instead of 58 and 42, and the drain -- bound by each SM's 30 B/clk
-                // store path while the tensor pipe waits -- is as long as its longer half.
+                // turned around in registers and put where CTA 0 would have put it (the slot layout does not change).  Both CTAs
+                // then drain 50 chunks instead of 58 and 42, and the drain -- bound by each SM's 30 B/clk store path while the
+                // tensor pipe waits -- is as long as its longer half.
                 const bool diag = (seg.I == seg.J);
                 const int ra_begin = diag ? row0 : 0;
                 const int ra_end = (diag && rank == 0) ? min(cols_valid, kDiagSplitCol) : cols_valid;
