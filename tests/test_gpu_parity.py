@@ -95,6 +95,19 @@ def test_edge_shapes_exact(xb, n, f, t, kind):
     assert np.array_equal(run_gpu(xb, [fr]), oracle.planar(fr))
 
 
+# The symmetric block G[0:128, 128:256] of a diagonal super-tile is written half by each CTA of the pair, CTA 1's half turned
+# around in registers (xengine_kernel.cuh, epilogue): input counts around the split column 192 and the block edges, so that
+# CTA 1 has none, part or all of its rows 192..255 -- as one frame (plain stores) and as two added frames (staging buffer +
+# bulk reduce-add), on one-tile shapes and with a ragged last diagonal tile behind an off-diagonal one.
+@pytest.mark.parametrize("n", [176, 192, 208, 224, 240, 256, 448, 480, 512])
+@pytest.mark.parametrize("frames", [1, 2])
+def test_shared_symmetric_block_at_ragged_input_counts(xb, n, frames):
+    f, t = 3, 200
+    frs = [wl.make_frame("uniform" if k == 0 else "gaussian", n, f, t, seed=5 * n + k) for k in range(frames)]
+    want = sum(oracle.planar(fr).astype(np.int64) for fr in frs)
+    assert np.array_equal(run_gpu(xb, frs), want)
+
+
 # Shapes whose schedule (xcorr_debug_schedule at this GPU's worker count) gives EVERY worker several segments, so the
 # accumulator hand-off between segments (TMEM full/empty phases), the TMA prologue crossing a segment boundary, the
 # water-filled split of an item along time and, for N > 256, diagonal <-> off-diagonal transitions inside one worker are
