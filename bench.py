@@ -449,12 +449,12 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.15)            # (the sampler's first reading; before the warm-up so that nothing idles between it and the timed steps)
     for k in range(warm):
         r.step(k)
     barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    time.sleep(0.15)
     # -- timed region 1: K whole steps, CUDA events on the launching stream
     launches0 = x.kernel_launches
     total_ms = r.timed_steps(steps, barrier)
