@@ -485,6 +485,8 @@ def main():
     roofline = tensor_roofline(cfg, k_ms, peaks, ceiling)
     roofline["kernel_ms_min"] = min(kern_ms)
     roofline["peak_source"] = f"2 x bf16_tflops (burst) of MEASURED_PEAKS.json [{peaks['source']}]; int8:bf16 nominal ratio 4.5:2.25"
+    roofline["note"] = ("frac may exceed 1: the peak is another dtype's MEASURED library GEMM rate (cuBLAS bf16) x the nominal int8:bf16 ratio, "
+                        "which understates the int8 pipe; frac_useful_of_issue_ceiling is against the measured issue rate of the int8 pipe itself")
     if ceiling:
         roofline["int8_issue_ceiling"] = ceiling
     elif rank == 0 and not args.no_int8_probe:
