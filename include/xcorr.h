@@ -56,6 +56,7 @@ extern "C" {
 #define XCORR_ENOMEM     -3   /* device or host allocation failed */
 #define XCORR_ECUDA      -4   /* a CUDA runtime/driver call failed; xcorr_last_cuda_error() has the code */
 #define XCORR_EOVERFLOW  -5   /* this frame could push an int32 sum past 2^31-1; nothing was launched */
+#define XCORR_ELIMIT     -6   /* larger than a built-in, never-allocated scratch table (xcorr_assemble_static); nothing was launched */
 
 typedef struct xcorr_handle xcorr_handle;
 typedef struct xcorr_stream xcorr_stream;

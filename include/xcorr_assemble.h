@@ -103,6 +103,68 @@ int xcorr_assemble(xcorr_assembler *a, const void *packets, size_t n_packets, ui
 int xcorr_assemble_accounted(xcorr_assembler *a, xcorr_handle *h, const void *packets, size_t n_packets, uint64_t seq0,
                              void *frame_dev, uint8_t *flags_dev, int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream);
 
+/*
+ * xcorr_assemble_static -- xcorr_assemble() for callers that must not allocate.  Same operation (PAPER.md:65-:81), same
+ * kernels, same outputs byte for byte; what differs is where the scratch memory lives.
+ *
+ * Who needs it.  The paper's pipeline allocates everything at start-up and nothing afterwards ("the entire application
+ * does not malloc or free any memory outside of startup and shutdown"), and a running acquisition has good
+ * reason: cudaMalloc and cudaFree serialise against the whole device, so one call from any thread stalls the
+ * correlation kernels of every stream in the middle of an integration.  A per-frame worker thread of such a pipeline
+ * that was never handed an xcorr_assembler (a stream added, a frame length changed while the system runs) has no
+ * permitted way to make one.  The other case is a process whose device memory is already spoken for by another
+ * allocator (a PyTorch caching pool that has taken the card, a fixed partition handed out by a supervisor): a driver
+ * allocation from inside this library can fail there or break the budget.  xcorr_assembler_create() allocates the position-ownership tables and the
+ * counters with cudaMalloc; this call needs neither a handle nor an allocation.
+ *
+ * How.  The ownership tables and counters sit in one array that is part of libxcorr.so's device image (a file-scope
+ * __device__ array of XCORR_ASSEMBLE_STATIC_SCRATCH_BYTES = 1 MiB + 256 B).  Every GPU on which the library's kernels
+ * get loaded holds that array until the process exits, whether this call is ever used or not.  It bounds the frame:
+ *
+ *     (T / S) * (F / C)  <=  XCORR_ASSEMBLE_STATIC_MAX_POSITIONS  (131072 packet positions per frame;
+ *                                                                   the paper's 256 MiB frame has 32768)
+ *
+ * A larger frame is refused with XCORR_ELIMIT before anything is enqueued; nothing is ever allocated to make it fit.
+ *
+ *   n_inputs, n_freq, t_per_frame, samples_per_packet, freq_per_packet
+ *               the shapes xcorr_assembler_create() takes, with the same rules (N % 16 == 0, T % S == 0, F % C == 0,
+ *               C * N a multiple of 128), checked on every call -- there is no handle to remember them.
+ *   packets, n_packets, seq0, frame_dev, flags_dev, lost_dev, counts_dev, cuda_stream
+ *               exactly as for xcorr_assemble(); all pointers belong to the CURRENT device.  The caller owns inputs and
+ *               outputs; the library owns only the built-in scratch.
+ *
+ * Per call, on `cuda_stream`: two cudaMemsetAsync (the part of the ownership table this frame uses -> "no owner", the
+ * counters -> 0), then packet_claim_kernel and assemble_kernel.  The call makes no cudaMalloc, cudaMallocHost,
+ * cudaFree, stream / event creation or any other allocating call, first call included, and builds no host tables.
+ *
+ * First call on a device.  It looks up the device address of the built-in array (cudaGetSymbolAddress -- the name of a
+ * __device__ array means nothing to host code until that is done, per device, with that device current), reads the SM
+ * count and checks the architecture, and remembers all three for the process's lifetime.  This forces the library's
+ * device code to be loaded onto that GPU if it was not yet.  Make this first call during start-up, and before any
+ * stream capture is begun: a frame with n_packets = 0 is enough.
+ *
+ * Shared state -- read this.  There is ONE scratch array per device, shared by every caller in the process, and it
+ * keeps whatever the last call left in it.  Each call clears what it needs at its own start, in stream order, so calls
+ * one after another on one stream, or on streams the caller has ordered with events, are independent of each other and
+ * of their shapes.  Two calls whose kernels may run at the same time on one GPU (different streams without such
+ * ordering, different host threads each on its own stream) trample each other's ownership tables and counters: the
+ * frames and counts that come out are garbage and nothing reports it.  Callers that need concurrent assembly on one GPU
+ * create one xcorr_assembler per stream at start-up instead.  xcorr_assembler handles have their own tables and are
+ * not affected by this call.
+ *
+ * Errors: EINVAL (shape rules, NULL / misaligned pointers, n_packets > 2^31 - 2), ELIMIT (more positions than the
+ * built-in table holds), EARCH (current device is not sm_100), ECUDA (xcorr_assemble_static_last_cuda_error() has the
+ * CUDA code).
+ */
+#define XCORR_ASSEMBLE_STATIC_MAX_POSITIONS 131072
+#define XCORR_ASSEMBLE_STATIC_SCRATCH_BYTES (2 * 4 * XCORR_ASSEMBLE_STATIC_MAX_POSITIONS + 256)
+int xcorr_assemble_static(int n_inputs, int n_freq, int t_per_frame, int samples_per_packet, int freq_per_packet,
+                          const void *packets, size_t n_packets, uint64_t seq0, void *frame_dev, uint8_t *flags_dev,
+                          int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream);
+
+/* CUDA error code behind the calling thread's most recent XCORR_ECUDA from xcorr_assemble_static (0 if none). */
+int xcorr_assemble_static_last_cuda_error(void);
+
 /* Total number of this library's kernels launched through the assembler so far. */
 uint64_t xcorr_assembler_kernel_launches(const xcorr_assembler *a);
 

@@ -13,7 +13,8 @@ from pathlib import Path
 from . import _build
 
 __all__ = [
-    "XCORR_OK", "XCORR_EINVAL", "XCORR_EARCH", "XCORR_ENOMEM", "XCORR_ECUDA", "XCORR_EOVERFLOW",
+    "XCORR_OK", "XCORR_EINVAL", "XCORR_EARCH", "XCORR_ENOMEM", "XCORR_ECUDA", "XCORR_EOVERFLOW", "XCORR_ELIMIT",
+    "XCORR_ASSEMBLE_STATIC_MAX_POSITIONS", "xcorr_assemble_static", "xcorr_assemble_static_last_cuda_error",
     "XCorrError", "lib", "xcorr_create", "xcorr_process", "xcorr_read", "xcorr_destroy", "xcorr_strerror",
     "xcorr_last_cuda_error", "xcorr_frame_bytes", "xcorr_output_bytes", "xcorr_kernel_launches",
     "xcorr_norm_enable", "xcorr_norm_process", "xcorr_read_normalized", "xcorr_promise_complete_frames",
@@ -24,7 +25,8 @@ __all__ = [
     "xcorr_debug_schedule", "xcorr_debug_stage_samples", "XCorr", "XCorrStream", "Assembler",
 ]
 
-XCORR_OK, XCORR_EINVAL, XCORR_EARCH, XCORR_ENOMEM, XCORR_ECUDA, XCORR_EOVERFLOW = 0, -1, -2, -3, -4, -5
+XCORR_OK, XCORR_EINVAL, XCORR_EARCH, XCORR_ENOMEM, XCORR_ECUDA, XCORR_EOVERFLOW, XCORR_ELIMIT = 0, -1, -2, -3, -4, -5, -6
+XCORR_ASSEMBLE_STATIC_MAX_POSITIONS = 131072   # include/xcorr_assemble.h
 
 _lib = None
 
@@ -99,6 +101,10 @@ def lib() -> ctypes.CDLL:
     L.xcorr_assemble.restype = ci
     L.xcorr_assemble_accounted.argtypes = [vp, vp, vp, ctypes.c_size_t, ctypes.c_uint64, vp, vp, vp, vp, vp]
     L.xcorr_assemble_accounted.restype = ci
+    L.xcorr_assemble_static.argtypes = [ci, ci, ci, ci, ci, vp, ctypes.c_size_t, ctypes.c_uint64, vp, vp, vp, vp, vp]
+    L.xcorr_assemble_static.restype = ci
+    L.xcorr_assemble_static_last_cuda_error.argtypes = []
+    L.xcorr_assemble_static_last_cuda_error.restype = ci
     L.xcorr_assembler_kernel_launches.argtypes = [vp]
     L.xcorr_assembler_kernel_launches.restype = ctypes.c_uint64
     L.xcorr_assembler_destroy.argtypes = [vp]
@@ -201,6 +207,23 @@ def xcorr_assemble_accounted(assembler: int, handle: int, packets: int, n_packet
                              lost_dev: int = 0, counts_dev: int = 0, cuda_stream: int = 0) -> int:
     return lib().xcorr_assemble_accounted(assembler, handle, packets or None, int(n_packets), int(seq0), frame_dev or None,
                                           flags_dev or None, lost_dev or None, counts_dev or None, cuda_stream)
+
+
+def xcorr_assemble_static(n_inputs: int, n_freq: int, t_per_frame: int, samples_per_packet: int, freq_per_packet: int, packets: int,
+                          n_packets: int, seq0: int, frame_dev: int, flags_dev: int = 0, lost_dev: int = 0, counts_dev: int = 0,
+                          cuda_stream: int = 0) -> int:
+    """xcorr_assemble without an assembler handle and without any allocation: for callers that must not allocate while the
+    system runs (per-frame threads of a live acquisition, processes whose device memory another allocator owns).  The
+    scratch is a fixed array inside libxcorr.so, so a frame may have at most XCORR_ASSEMBLE_STATIC_MAX_POSITIONS packet
+    positions (else XCORR_ELIMIT), and calls that overlap on one GPU race on it.  Make the first call on each device at
+    start-up.  Contract: include/xcorr_assemble.h."""
+    return lib().xcorr_assemble_static(int(n_inputs), int(n_freq), int(t_per_frame), int(samples_per_packet), int(freq_per_packet),
+                                       packets or None, int(n_packets), int(seq0), frame_dev or None, flags_dev or None,
+                                       lost_dev or None, counts_dev or None, cuda_stream)
+
+
+def xcorr_assemble_static_last_cuda_error() -> int:
+    return lib().xcorr_assemble_static_last_cuda_error()
 
 
 def xcorr_assembler_kernel_launches(assembler: int) -> int:

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -105,6 +106,7 @@ extern "C" const char *xcorr_strerror(int code)
         case XCORR_ENOMEM: return "out of memory";
         case XCORR_ECUDA: return "CUDA call failed (see xcorr_last_cuda_error)";
         case XCORR_EOVERFLOW: return "integration too long: an int32 visibility could overflow";
+        case XCORR_ELIMIT: return "frame has more packet positions than the built-in scratch table holds (xcorr_assemble_static)";
         default: return "unknown xcorr error code";
     }
 }
@@ -852,5 +854,126 @@ extern "C" int xcorr_stream_read_normalized(xcorr_stream *s, float *vis_out, int
     const int rc = xcorr_read_normalized(s->h, vis_out, lost_matrix_out, (void *)s->compute_stream);
     if (rc != XCORR_OK) return rc;
     XC_CUDA(s->h, cudaStreamSynchronize(s->compute_stream));
+    return XCORR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// xcorr_assemble_static: packet -> frame assembly with no allocation anywhere (include/xcorr_assemble.h)
+// ---------------------------------------------------------------------------------------------------
+// For callers that may not allocate (per-frame threads of a running acquisition -- a cudaMalloc would stall every
+// stream of the device mid-integration, PAPER.md:49 -- and processes whose device memory belongs to another
+// allocator).  The scratch that xcorr_assembler_create() gets from cudaMalloc is this array instead; it is part of the
+// library's device image, so every GPU that loads the image holds these bytes until the process ends.
+//
+//   words [0, kStaticMaxPos)               ownership table of the frame being assembled (cleared per call)
+//   words [kStaticMaxPos, 2 kStaticMaxPos) the table assemble_kernel resets for "the next frame": write-only here, since
+//                                          each call clears its own table and never relies on the previous call's state
+//   words [2 kStaticMaxPos, +8)            the packet counters counts[0..5] of assemble_kernel.cuh (cleared per call)
+//
+// One array per device, shared by all callers: calls that overlap on the GPU race on it (documented in the header).
+constexpr unsigned kStaticMaxPos = XCORR_ASSEMBLE_STATIC_MAX_POSITIONS;
+constexpr size_t kStaticScratchWords = 2 * (size_t)kStaticMaxPos + 64;
+static_assert(kStaticScratchWords * sizeof(uint32_t) == XCORR_ASSEMBLE_STATIC_SCRATCH_BYTES, "header and array disagree");
+static __device__ __align__(256) uint32_t g_static_assemble_scratch[kStaticScratchWords];
+
+// In host code `g_static_assemble_scratch` is only a handle for the runtime's symbol table, not memory the GPU can
+// reach under that address: the device address has to be asked for, per device, with that device current.
+constexpr int kStaticMaxDevices = 64;
+struct StaticDeviceState {
+    bool ready = false;
+    uint32_t *scratch = nullptr;   // device address of g_static_assemble_scratch on this device
+    int n_sms = 0;
+    int ctas_per_sm = 0;           // resident CTAs of assemble_kernel<false> (256 threads): the grid is one wave
+};
+static StaticDeviceState g_static_state[kStaticMaxDevices];
+static std::mutex g_static_mutex;
+static thread_local int g_static_last_cuda_error = 0;
+
+extern "C" int xcorr_assemble_static_last_cuda_error(void) { return g_static_last_cuda_error; }
+
+#define XC_STATIC_CUDA(expr)                              \
+    do {                                                  \
+        cudaError_t e_ = (expr);                          \
+        if (e_ != cudaSuccess) {                          \
+            cudaGetLastError();                           \
+            g_static_last_cuda_error = (int)e_;           \
+            return XCORR_ECUDA;                           \
+        }                                                 \
+    } while (0)
+
+// Once per device, `dev` current: architecture check, SM count, occupancy, device address of the scratch array.
+// None of these allocates on behalf of the caller; the symbol lookup makes the runtime load the library's device
+// image onto this GPU if no kernel of it has run here yet (which is why the first call belongs to start-up).
+static int static_assemble_setup(int dev, StaticDeviceState *out)
+{
+    std::lock_guard<std::mutex> guard(g_static_mutex);
+    StaticDeviceState &st = g_static_state[dev];
+    if (!st.ready) {
+        int major = 0, n_sms = 0, ctas = 0;
+        XC_STATIC_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        if (major != 10) return XCORR_EARCH;
+        XC_STATIC_CUDA(cudaDeviceGetAttribute(&n_sms, cudaDevAttrMultiProcessorCount, dev));
+        XC_STATIC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, assemble_kernel<false>, 256, 0));
+        void *addr = nullptr;
+        XC_STATIC_CUDA(cudaGetSymbolAddress(&addr, g_static_assemble_scratch));
+        if (!addr || n_sms < 1 || ctas < 1) { g_static_last_cuda_error = (int)cudaErrorUnknown; return XCORR_ECUDA; }
+        st.scratch = static_cast<uint32_t *>(addr);
+        st.n_sms = n_sms;
+        st.ctas_per_sm = ctas;
+        st.ready = true;
+    }
+    *out = st;
+    return XCORR_OK;
+}
+
+extern "C" int xcorr_assemble_static(int n_inputs, int n_freq, int t_per_frame, int samples_per_packet, int freq_per_packet,
+                                     const void *packets, size_t n_packets, uint64_t seq0, void *frame_dev, uint8_t *flags_dev,
+                                     int32_t *lost_dev, uint32_t *counts_dev, void *cuda_stream)
+{
+    // the checks of xcorr_assembler_create and of xcorr_assemble, on every call: there is no handle to remember a shape
+    int rc = validate_shape(n_inputs, n_freq, t_per_frame);
+    if (rc != XCORR_OK) return rc;
+    const int S = samples_per_packet, C = freq_per_packet;
+    if (S <= 0 || C <= 0 || t_per_frame % S != 0 || n_freq % C != 0) return XCORR_EINVAL;
+    if (((long long)C * n_inputs) % 128 != 0) return XCORR_EINVAL;
+    if (!frame_dev || (!packets && n_packets) || n_packets > 0x7FFFFFFEull) return XCORR_EINVAL;
+    if (((uintptr_t)packets & 15u) || ((uintptr_t)frame_dev & 15u) || ((uintptr_t)flags_dev & 15u) || ((uintptr_t)lost_dev & 3u) ||
+        ((uintptr_t)counts_dev & 3u))
+        return XCORR_EINVAL;
+    AssembleShape sh = {};
+    sh.n_inputs = n_inputs; sh.n_freq = n_freq; sh.n_time = t_per_frame;
+    sh.s_per_packet = S; sh.c_per_packet = C;
+    sh.n_streams = n_freq / C; sh.n_blocks = t_per_frame / S;
+    const unsigned long long pay = (unsigned long long)S * C * n_inputs;
+    sh.packet_bytes = kPacketHeaderBytes + pay + pay / 8;
+    const unsigned long long n_pos64 = (unsigned long long)sh.n_streams * (unsigned long long)sh.n_blocks;
+    if (n_pos64 == 0) return XCORR_EINVAL;
+    if (n_pos64 > kStaticMaxPos) return XCORR_ELIMIT;   // the table is what it is: never grown, nothing allocated instead
+    const unsigned n_pos = (unsigned)n_pos64;
+
+    int dev = -1;
+    XC_STATIC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return XCORR_EINVAL;
+    StaticDeviceState st;
+    if ((rc = static_assemble_setup(dev, &st)) != XCORR_OK) return rc;
+
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    uint32_t *owner = st.scratch;                        // this frame's claims
+    uint32_t *owner_sink = st.scratch + kStaticMaxPos;   // assemble_kernel's reset of "the other table": unused here
+    uint32_t *counts = st.scratch + 2 * (size_t)kStaticMaxPos;
+    // the array holds whatever the last call (any shape, any caller) left there: start from "no owner" and zero counters
+    XC_STATIC_CUDA(cudaMemsetAsync(owner, 0xFF, sizeof(uint32_t) * (size_t)n_pos, s));
+    XC_STATIC_CUDA(cudaMemsetAsync(counts, 0, sizeof(uint32_t) * 8, s));
+    {
+        const size_t n_threads = n_packets > (size_t)n_freq ? n_packets : (size_t)n_freq;   // also zeroes lost_dev[F]
+        packet_claim_kernel<<<(unsigned)((n_threads + 255) / 256), 256, 0, s>>>((const uint8_t *)packets, (unsigned)n_packets, seq0, sh, owner,
+                                                                               counts, lost_dev);
+        XC_STATIC_CUDA(cudaGetLastError());
+    }
+    unsigned blocks = (unsigned)st.n_sms * (unsigned)st.ctas_per_sm;
+    if (blocks > n_pos) blocks = n_pos;
+    assemble_kernel<false><<<blocks, 256, 0, s>>>((const uint8_t *)packets, sh, owner, owner_sink, (uint8_t *)frame_dev, flags_dev, lost_dev,
+                                                  counts, counts_dev, nullptr, nullptr, nullptr);
+    XC_STATIC_CUDA(cudaGetLastError());
     return XCORR_OK;
 }
