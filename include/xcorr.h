@@ -33,8 +33,11 @@
  *     previous call first makes that stream wait, on the device (cudaStreamWaitEvent), for everything enqueued so far
  *     on the previous stream -- so xcorr_process on stream A followed by xcorr_read on stream B is safe and exact.  A
  *     stream handed to a call must therefore stay alive until the handle's next call has returned (or the handle is
- *     destroyed); if CUDA reports the previous stream as invalid the call returns XCORR_EINVAL.  The host-side
- *     bookkeeping (first frame of an integration, overflow guard, sample count) follows the order of the CALLS.
+ *     destroyed).  Destroying it earlier is undefined behaviour, as for any CUDA call on a dead stream: the next call
+ *     records an event on it.  Where CUDA happens to report the stream as invalid the call returns XCORR_EINVAL, but
+ *     that is a courtesy, not a contract.  (The Python wrappers keep the last stream object referenced for this reason.)
+ *     The host-side bookkeeping (first frame of an integration, overflow guard, sample count) follows the order of the
+ *     CALLS.
  *   - Nothing is allocated or freed after xcorr_create()/xcorr_stream_create() return (PAPER.md:49:
  *     "the entire application does not malloc or free any memory outside of startup and shutdown").
  *   - There is no CPU fallback: on a machine without an sm_100 GPU xcorr_create() fails with
@@ -156,7 +159,8 @@ int xcorr_norm_enable(xcorr_handle *h);
  *   lost_samples_host  HOST pointer, int32[F]: time samples of each channel lost with their packets in this
  *                      frame (0 <= value <= T; the paper's packet-loss counter, kept per channel: a stream's
  *                      counter applies to its 8 channels).  Read before the call returns.
- * Errors: EINVAL (normalisation not enabled, misaligned, counter out of range), ECUDA.
+ * Errors: EINVAL (normalisation not enabled, misaligned, counter out of range), ECUDA.  A call that fails has counted
+ * nothing (neither flags nor lost samples), so it can be repeated as a whole.
  */
 int xcorr_norm_process(xcorr_handle *h, const uint8_t *flags_dev, const int32_t *lost_samples_host, void *cuda_stream);
 

@@ -324,6 +324,13 @@ class XCorr:
     def kernel_launches(self) -> int:
         return xcorr_kernel_launches(self.handle)
 
+    def _stream(self, stream) -> int:
+        """The cudaStream_t of ``stream``; keeps the stream OBJECT referenced until this handle's next call has been given its
+        own: the library records an event on the previous call's stream at the next call (stream order, include/xcorr.h),
+        so that stream must not be destroyed by Python's garbage collector in between."""
+        self._prev_stream, self._last_stream = getattr(self, "_last_stream", None), stream   # the previous one lives through this call
+        return _stream_handle(stream)
+
     def _check(self, rc: int, what: str):
         if rc != XCORR_OK:
             raise XCorrError(rc, what, xcorr_last_cuda_error(self.handle))
@@ -332,7 +339,7 @@ class XCorr:
         """frame_dev: torch uint8 CUDA tensor of N*F*T bytes ([T][F][N]), contiguous."""
         if not frame_dev.is_cuda or not frame_dev.is_contiguous() or frame_dev.numel() * frame_dev.element_size() != self.frame_bytes:
             raise ValueError("frame_dev must be a contiguous CUDA tensor of exactly frame_bytes bytes")
-        self._check(xcorr_process(self.handle, frame_dev.data_ptr(), _stream_handle(stream)), "xcorr_process")
+        self._check(xcorr_process(self.handle, frame_dev.data_ptr(), self._stream(stream)), "xcorr_process")
 
     def read(self, out=None, stream=None):
         """Write int32[F][P][2] into ``out`` (CUDA or CPU torch int32 tensor; allocated on the device if None)."""
@@ -341,7 +348,7 @@ class XCorr:
             out = torch.empty((self.n_freq, self.n_pairs, 2), dtype=torch.int32, device="cuda")
         if out.dtype != torch.int32 or not out.is_contiguous() or out.numel() * 4 != self.output_bytes:
             raise ValueError("out must be a contiguous int32 tensor of output_bytes bytes")
-        self._check(xcorr_read(self.handle, out.data_ptr(), _stream_handle(stream)), "xcorr_read")
+        self._check(xcorr_read(self.handle, out.data_ptr(), self._stream(stream)), "xcorr_read")
         return out
 
     def promise_complete_frames(self, enabled: bool = True) -> None:
@@ -366,7 +373,7 @@ class XCorr:
             if lost_samples.shape != (self.n_freq,):
                 raise ValueError("lost_samples must have shape (n_freq,)")
             lptr = lost_samples.ctypes.data
-        self._check(xcorr_norm_process(self.handle, fptr, lptr, _stream_handle(stream)), "xcorr_norm_process")
+        self._check(xcorr_norm_process(self.handle, fptr, lptr, self._stream(stream)), "xcorr_norm_process")
 
     def norm_process_dev(self, flags_dev=None, lost_dev=None, stream=None) -> None:
         """As norm_process with the packet-loss counters in a CUDA int32 tensor [F] (the output of Assembler.assemble)."""
@@ -376,7 +383,7 @@ class XCorr:
         if lost_dev is not None and (not lost_dev.is_cuda or lost_dev.numel() != self.n_freq or lost_dev.element_size() != 4):
             raise ValueError("lost_dev must be a CUDA int32 tensor of n_freq elements")
         lptr = lost_dev.data_ptr() if lost_dev is not None else 0
-        self._check(xcorr_norm_process_dev(self.handle, fptr, lptr, _stream_handle(stream)), "xcorr_norm_process_dev")
+        self._check(xcorr_norm_process_dev(self.handle, fptr, lptr, self._stream(stream)), "xcorr_norm_process_dev")
 
     def read_normalized(self, out=None, lost_out=None, stream=None):
         """-> float32[F][P][2] (allocated on the device if None); lost_out: optional int32[F][P] tensor for L."""
@@ -390,7 +397,7 @@ class XCorr:
             if lost_out.dtype != torch.int32 or not lost_out.is_contiguous() or lost_out.numel() * 8 != self.output_bytes:
                 raise ValueError("lost_out must be a contiguous int32 tensor of n_freq * n_pairs elements")
             lptr = lost_out.data_ptr()
-        self._check(xcorr_read_normalized(self.handle, out.data_ptr(), lptr, _stream_handle(stream)), "xcorr_read_normalized")
+        self._check(xcorr_read_normalized(self.handle, out.data_ptr(), lptr, self._stream(stream)), "xcorr_read_normalized")
         return out
 
     def close(self) -> None:
@@ -509,7 +516,7 @@ class Assembler:
                                 _stream_handle(stream))
         else:
             rc = xcorr_assemble_accounted(self.handle, account_into.handle, pptr, n_packets, seq0, frame.data_ptr(), flags.data_ptr(),
-                                          lost.data_ptr(), counts.data_ptr(), _stream_handle(stream))
+                                          lost.data_ptr(), counts.data_ptr(), account_into._stream(stream))
         if rc != XCORR_OK:
             raise XCorrError(rc, "xcorr_assemble")
         return frame, flags, lost, counts

@@ -65,8 +65,8 @@ __device__ __forceinline__ void mbar_arrive_local(uint32_t bar)
     asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 // arrive on a barrier given by a shared::cluster address (own or peer CTA).  Default .release.cta semantics on
-// purpose: a cluster-scope release costs MEMBAR.ALL.GPU + ERRBAR per arrive (measured: 18 % of all stall samples,
-// profiles/r01_dev_notes.md); the data handed over lives in the arriving CTA's own smem and is published to the
+// purpose: a cluster-scope release costs MEMBAR.ALL.GPU + ERRBAR per arrive (measured in round 1: 18 % of all stall
+// samples of the kernel); the data handed over lives in the arriving CTA's own smem and is published to the
 // tensor core by fence.proxy.async, the arrive itself is only the signal.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster_addr)
 {
@@ -218,12 +218,6 @@ __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.
 __device__ __forceinline__ void st_global_v4(int32_t *addr, int32_t a, int32_t b, int32_t c, int32_t d)
 {
     asm volatile("st.global.v4.s32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
-}
-__device__ __forceinline__ int4 ld_global_v4(const int32_t *addr)
-{
-    int4 r;
-    asm volatile("ld.global.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(addr) : "memory");
-    return r;
 }
 
 // ---------------------------------------------------------------- bulk (TMA) reduce smem -> global, issued by one thread

@@ -519,18 +519,23 @@ extern "C" int xcorr_norm_process(xcorr_handle *h, const uint8_t *flags_dev, con
 {
     if (!h || !h->norm) return XCORR_EINVAL;
     if (flags_dev && ((uintptr_t)flags_dev & 15u) != 0) return XCORR_EINVAL;
-    if (lost_samples_host) {
+    if (lost_samples_host)
         for (int f = 0; f < h->n_freq; ++f)
             if (lost_samples_host[f] < 0 || lost_samples_host[f] > h->n_time) return XCORR_EINVAL;
-        for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] += lost_samples_host[f];
-        h->lost_host_dirty = true;
-    }
     if (flags_dev) {
         int rc = check_device(h->device);
         if (rc != XCORR_OK) return rc;
         if ((rc = order_after_previous(h, (cudaStream_t)cuda_stream)) != XCORR_OK) return rc;
     }
-    return launch_flag_count(h, flags_dev, cuda_stream);
+    // the flag launch goes first: if it fails, the host-side loss counters have not moved and the caller may retry the
+    // whole call without counting this frame's lost samples twice
+    const int rc = launch_flag_count(h, flags_dev, cuda_stream);
+    if (rc != XCORR_OK) return rc;
+    if (lost_samples_host) {
+        for (int f = 0; f < h->n_freq; ++f) h->lost_acc[f] += lost_samples_host[f];
+        h->lost_host_dirty = true;
+    }
+    return XCORR_OK;
 }
 
 static int launch_flag_count(xcorr_handle *h, const uint8_t *flags_dev, void *cuda_stream)
@@ -782,7 +787,19 @@ static int assemble_common(xcorr_assembler *a, xcorr_handle *h, const void *pack
     else
         assemble_kernel<false><<<blocks, 256, 0, s>>>((const uint8_t *)packets, a->sh, owner, owner_next, (uint8_t *)frame_dev, flags_dev,
                                                       lost_dev, a->counts, counts_dev, nullptr, nullptr, nullptr);
-    XC_CUDA(a, cudaGetLastError());
+    {
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) {
+            // packet_claim_kernel is in the stream and has dirtied this call's table and the counters, but nothing will clean
+            // them (that is assemble_kernel's job and `calls` does not advance): put the "all clean on entry" state back by
+            // hand so that a later call does not read this frame's owners as its own
+            a->last_cuda_error = (int)e;
+            cudaMemsetAsync(a->owner, 0xFF, sizeof(uint32_t) * 2 * (size_t)a->n_positions, s);
+            cudaMemsetAsync(a->counts, 0, sizeof(uint32_t) * 8, s);
+            cudaGetLastError();
+            return XCORR_ECUDA;
+        }
+    }
     a->launches += 1;
     a->calls += 1;   // the tables swap roles only once both kernels are in the stream
     if (h) {

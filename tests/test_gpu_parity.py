@@ -370,7 +370,7 @@ def test_c4_full_size(xb):
     got = run_gpu(xb, [fr])
     # whole channels against the oracle: 0 and 7 from the data-parallel part of the schedule (items that run whole on one
     # worker), 14 and 15 from the water-filled remainder (items cut in time, up to 9 segments per worker)
-    seg, wb = xb.xcorr_debug_schedule(c.n_inputs, c.n_freq, c.n_time, 74)
+    seg, wb = xb.xcorr_debug_schedule(c.n_inputs, c.n_freq, c.n_time, n_workers())
     n_stage = -(-c.n_time // xb.xcorr_debug_stage_samples())
     whole = {int(s[0]) for s in seg if s[4] - s[3] == n_stage}
     cut = {int(s[0]) for s in seg if s[4] - s[3] < n_stage}
@@ -515,6 +515,28 @@ def test_process_and_read_on_different_streams_are_ordered(xb):
     want2 = oracle.planar(frames[2])
     for k, o in enumerate(outs):
         assert np.array_equal(o.cpu().numpy(), want01 if k % 2 == 0 else want2), k
+    x.close()
+
+
+def test_wrapper_keeps_a_temporary_stream_alive_until_the_next_call(xb):
+    """include/xcorr.h: the stream of a call must outlive the handle's next call (that call records an event on it).  A
+    torch stream created for one ``process`` and dropped at once would break that; ``XCorr`` keeps the object referenced."""
+    import gc
+    n, f, t = 64, 16, 256
+    frames = [wl.uniform_frame(n, f, t, seed=8200 + k) for k in range(2)]
+    dev = [torch.from_numpy(fr).cuda() for fr in frames]
+    torch.cuda.synchronize()
+    x = xb.XCorr(n, f, t)
+    keep = torch.cuda.Stream()
+    for rep in range(3):
+        x.process(dev[0], torch.cuda.Stream())     # temporary: no other reference than the wrapper's
+        gc.collect()
+        assert isinstance(x._last_stream, torch.cuda.Stream)
+        x.process(dev[1], torch.cuda.Stream())
+        gc.collect()
+        got = x.read(None, keep)
+        torch.cuda.synchronize()
+        assert np.array_equal(got.cpu().numpy(), oracle.planar(frames[0]).astype(np.int64) + oracle.planar(frames[1]))
     x.close()
 
 
