@@ -14,7 +14,7 @@ two of them alternating), so no flush is needed between iterations.
 Beside the K timed steps the line carries a `sustained` leg (the same step back to back for >= 2 s with the clocks sampled
 during that leg only: the power-capped steady state), `other_configs` (C3: the 64-frame streamed run of BASELINE.json
 configs[2] in Gb/s with its H2D-only ceiling; C4, C5: step and kernel times, useful and issued int8 TOP/s) and the
-measured int8 issue ceiling of the tensor pipe (paper_1503_06189_b200/probe.py) as roofline.int8_issue_ceiling_tops.
+measured int8 issue ceiling of the tensor pipe (bench_support/probe.py) as roofline.int8_issue_ceiling_tops.
 
 Multi-GPU: the path does not shard ("replicas only"): --gpus N (under torchrun) runs N independent
 replicas, one per GPU, no collective on the data path; value = N frames' bits / max-over-ranks time.
@@ -421,7 +421,8 @@ def main():
 
     import torch
     import paper_1503_06189_b200 as xb
-    from paper_1503_06189_b200 import probe, replicas
+    from bench_support import probe
+    from paper_1503_06189_b200 import replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))

@@ -11,7 +11,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
-#include "../ptx.cuh"
+#include "../paper_1503_06189_b200/csrc/ptx.cuh"
 
 namespace {
 

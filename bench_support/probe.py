@@ -1,6 +1,7 @@
 """Measurement support (not on the product path): the resident-operand int8 tensor issue-rate probe.
 
-``libxcorr_probe.so`` is a separate library (csrc/probe/int8_issue_probe.cu); libxcorr.so does not contain it.  bench.py
+``libxcorr_probe.so`` is a separate library (bench_support/int8_issue_probe.cu, built here beside bench.py); libxcorr.so does
+not contain it and the product package does not import it.  It shares only the inline-PTX wrappers of csrc/ptx.cuh.  bench.py
 calls ``int8_issue_ceiling`` to fix the roofline denominator of xengine_kernel on the box it runs on.
 """
 from __future__ import annotations
@@ -10,9 +11,10 @@ import os
 import subprocess
 from pathlib import Path
 
-PKG = Path(__file__).resolve().parent
-SRC = PKG / "csrc" / "probe" / "int8_issue_probe.cu"
-LIB = PKG / "libxcorr_probe.so"
+HERE = Path(__file__).resolve().parent
+PKG = HERE.parent / "paper_1503_06189_b200"
+SRC = HERE / "int8_issue_probe.cu"
+LIB = HERE / "libxcorr_probe.so"
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared", "-Xcompiler", "-fPIC"]
 OPS_PER_MMA = 2 * 256 * 256 * 32
 

@@ -47,7 +47,7 @@ def test_library_exports_only_the_declared_c_abi():
 
 def test_support_libraries_build_and_export():
     """The two non-product libraries build for sm_100a without a GPU and export their one entry point each."""
-    from paper_1503_06189_b200 import probe
+    from bench_support import probe
     from tests import support
     assert probe.lib().xcorr_probe_int8_issue is not None
     assert support.lib().simt_xcorr is not None
