@@ -11,10 +11,16 @@ HBM; `e2e` is the same metric through the streamed C-ABI path (row a5) with page
 result, copies inside the timed region.  Inputs are synthetic (workloads.py) and larger than L2 (256 MiB frames,
 two of them alternating), so no flush is needed between iterations.
 
-Beside the K timed steps the line carries a `sustained` leg (the same step back to back for >= 2 s with the clocks sampled
-during that leg only: the power-capped steady state), `other_configs` (C3: the 64-frame streamed run of BASELINE.json
-configs[2] in Gb/s with its H2D-only ceiling; C4, C5: step and kernel times, useful and issued int8 TOP/s) and the
-measured int8 issue ceiling of the tensor pipe (bench_support/probe.py) as roofline.int8_issue_ceiling_tops.
+Two legs.  A B200 runs xengine_kernel at its 1965 MHz boost for a few milliseconds and then sits at the 1 kW power cap near
+1.5 GHz, so K steps from a cool part flatter.  The line's `value`, `ms_per_step`, `clocks` and `roofline` therefore come from
+exactly K steps timed directly behind a power-steady leg (the same step back to back for >= 2 s, counted in `warmup`); the K
+steps from a cool part are kept as `roofline.burst`.  `roofline.peak` is the issue ceiling of the int8 tensor pipe measured in
+the same run (bench_support/probe.py; sustained reading for the steady leg, burst reading for the burst leg); 2 x the
+measured cuBLAS bf16 rate is beside it as `frac_of_2x_bf16`.  `roofline` also carries what the driver's record must keep:
+the added-frame launches (frames added to a running integration, no read in between -- the telescope's steady state,
+PAPER.md:99), the long leg's figures (`sustained_*`) and a compact `configs` table of C3 / C4 / C5.  `other_configs` has
+their full entries (C3: the 64-frame streamed run of BASELINE.json configs[2] with its H2D-only ceiling; an oracle timing
+beside each), `cpu_baseline.one_core` the oracle on one core.
 
 Multi-GPU: the path does not shard ("replicas only"): --gpus N (under torchrun) runs N independent
 replicas, one per GPU, no collective on the data path; value = N frames' bits / max-over-ranks time.
@@ -135,6 +141,35 @@ def oracle_sample(cfg: wl.Config, fr=None):
             "sample": f"oracle.planar (plain C, int64 accumulators, OpenMP) on {n_ch} of {cfg.n_freq} channels x "
                       f"{t_samp} of {cfg.n_time} samples of one {cfg.name} frame (N={cfg.n_inputs}); {dt:.2f} s",
             "cmac_per_s": cmacs / dt, "seconds": dt}
+
+
+def oracle_one_core(cfg: wl.Config):
+    """The oracle, as it stands, on ONE host core: a child process with OMP_NUM_THREADS=1 (the thread count is fixed when the
+    OpenMP runtime starts) timing oracle.planar on a few whole channels of one frame; scaled per complex MAC."""
+    n_ch = max(1, min(cfg.n_freq, 4 if cfg.n_inputs <= 256 else 1))
+    t_samp = cfg.n_time if cfg.n_inputs <= 256 else min(cfg.n_time, 2048)
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        out = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--oracle-sample", f"{cfg.name}:{n_ch}:{t_samp}"], env=env,
+                             capture_output=True, text=True, timeout=300, check=True).stdout
+        d = json.loads(out.strip().splitlines()[-1])
+    except Exception as e:
+        return {"error": str(e)[:160]}
+    whole = cfg.cmacs_per_frame / d["cmac_per_s"]
+    d["whole_frame_seconds_scaled"] = whole
+    d["value_scaled"] = 8.0 * cfg.frame_bytes / whole / 1e9
+    d["scaling"] = "per complex MAC: whole frame = sample time x (F*T) / (channels*samples of the sample)"
+    return d
+
+
+def oracle_sample_cli(spec: str):
+    name, n_ch, t_samp = spec.split(":")
+    cfg = wl.CONFIGS[name]
+    import oracle
+    oracle.build()
+    fr = wl.make_frame(cfg.kind, cfg.n_inputs, int(n_ch), int(t_samp), cfg.seed)
+    d = oracle_sample(cfg, fr)
+    print(json.dumps({k: d[k] for k in ("value", "unit", "cores", "sample", "cmac_per_s", "seconds")}), flush=True)
 
 
 def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
@@ -306,36 +341,78 @@ class Resident:
         barrier()
         return [a.elapsed_time(b) for a, b in evs]
 
+    def timed_added(self, n, barrier):
+        """Frames ADDED to a running integration (the kernels "simply add to the output of the last run", no read in
+        between): one first frame, then n launches -> (per-launch xengine_kernel ms from events around each launch,
+        ms per launch of the same n launches back to back between two events)."""
+        torch = self.torch
+        self.x.read(self.out_dev, self.st)
+        self.x.process(self.dev_frames[0], self.st)                      # first frame of the integration (stores)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        for k in range(n):
+            evs[k][0].record(self.st)
+            self.x.process(self.dev_frames[(k + 1) % self.n_distinct], self.st)
+            evs[k][1].record(self.st)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(self.st)
+        for k in range(n):
+            self.x.process(self.dev_frames[k % self.n_distinct], self.st)
+        e1.record(self.st)
+        barrier()
+        self.x.read(self.out_dev, self.st)
+        barrier()
+        return [a.elapsed_time(b) for a, b in evs], e0.elapsed_time(e1) / n
+
     def close(self):
         self.x.close()
         self.dev_frames = self.host_frames = None
 
 
-def tensor_roofline(cfg, k_ms, peaks, ceiling=None):
-    """Tensor roofline entries of xengine_kernel for one launch of `cfg` taking k_ms."""
+def kstats(ms):
+    """mean / median / best of a list of per-launch durations (ms)."""
+    return {"mean": statistics.mean(ms), "median": statistics.median(ms), "min": min(ms), "launches": len(ms)}
+
+
+def added_frames_fit(cfg, n):
+    """2 n + 1 frames must stay inside the int32 guard of one integration (16,777,215 samples, include/xcorr.h)."""
+    return max(4, min(n, (16777215 // cfg.n_time - 1) // 2))
+
+
+TRAFFIC_SOURCE = {"C2": "profiles/r02_ncu_full_bench_c2.md", "C4": "profiles/r02_ncu_full_bench_c4_c5.md",
+                  "C5": "profiles/r02_ncu_full_bench_c4_c5.md"}
+
+
+def tensor_roofline(cfg, k_ms, peaks, ceiling=None, leg="sustained"):
+    """Tensor roofline entries of xengine_kernel for one launch of `cfg` taking k_ms.  `peak` is the issue ceiling of the int8
+    tensor pipe measured in this run on this box (bench_support/probe.py: resident operands, nothing but tcgen05.mma kind::i8) --
+    its sustained reading for a kernel timed inside a long, power-steady leg, its burst reading for a kernel timed from a cool
+    part.  Without the probe (--no-int8-probe) the stand-in is 2 x the measured cuBLAS bf16 rate of MEASURED_PEAKS.json."""
     alg_ops = 8.0 * cfg.cmacs_per_frame              # 4 real MACs = 8 int8 ops per complex MAC, useful pairs i<=j only
     achieved = alg_ops / (k_ms * 1e-3) / 1e12
-    peak = 2.0 * peaks["bf16_burst"]
-    peak_sustained = 2.0 * peaks["bf16_sustained"] if peaks.get("bf16_sustained") else None
-    iou = issued_over_useful(cfg)
-    r = {"bound": "tensor", "kernel": "xengine_kernel (xcorr_process)", "achieved": achieved, "peak": peak, "unit": "TOP/s",
-         "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "kernel_ms": k_ms, "algorithmic_ops_per_launch": alg_ops,
-         "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
-         "frac_of_sustained_peak": (achieved / peak_sustained) if peak_sustained else None, "peak_sustained": peak_sustained,
-         "issued_over_useful": iou, "issued_int8_tops": achieved * iou,
-         "hbm_gbs_staging": cfg.frame_bytes / (k_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]}
+    bf16 = peaks["bf16_sustained"] if (leg == "sustained" and peaks.get("bf16_sustained")) else peaks["bf16_burst"]
     if ceiling:
-        r["int8_issue_ceiling_tops"] = ceiling["burst_tops"]
-        r["frac_useful_of_issue_ceiling"] = achieved / ceiling["burst_tops"]
-        r["frac_issued_of_issue_ceiling"] = achieved * iou / ceiling["burst_tops"]
-    return r
+        peak = ceiling["sustained_tops" if leg == "sustained" else "burst_tops"]
+        source = f"int8 issue ceiling measured in this run ({leg} reading of bench_support/probe.py)"
+    else:
+        peak = 2.0 * bf16
+        source = f"2 x bf16_tflops ({leg}) of MEASURED_PEAKS.json [{peaks['source']}] x the nominal int8:bf16 ratio 4.5:2.25 (no probe in this run)"
+    iou = issued_over_useful(cfg)
+    return {"bound": "tensor", "kernel": "xengine_kernel (xcorr_process)", "achieved": achieved, "peak": peak, "unit": "TOP/s",
+            "frac": achieved / peak, "leg": leg, "peak_source": source,
+            "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "traffic_source": TRAFFIC_SOURCE.get(cfg.name),
+            "kernel_ms": k_ms, "algorithmic_ops_per_launch": alg_ops,
+            "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
+            "frac_of_2x_bf16": achieved / (2.0 * bf16), "peak_2x_bf16": 2.0 * bf16,
+            "issued_over_useful": iou, "issued_int8_tops": achieved * iou, "frac_issued_of_peak": achieved * iou / peak,
+            "hbm_gbs_staging": cfg.frame_bytes / (k_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]}
 
 
 C3_POOL = 4     # distinct seeded frames the 64-frame streamed run cycles through (1 GiB each, page-locked)
 
 
-def measure_other_config(name, xb, torch, peaks, ceiling, steps=20):
-    """C4 / C5 (device-resident step) and C3 (device-resident step + the 64-frame streamed run of BASELINE.json configs[2])."""
+def measure_other_config(name, xb, torch, peaks, ceiling, steps=20, min_seconds=1.0, cpu=True):
+    """C4 / C5 (device-resident step) and C3 (device-resident step + the 64-frame streamed run of BASELINE.json configs[2]).
+    The step leg runs for at least `min_seconds` (power-steady); the per-launch kernel times are taken straight behind it."""
     cfg = wl.CONFIGS[name]
     r = Resident(cfg, xb, torch)
 
@@ -344,25 +421,26 @@ def measure_other_config(name, xb, torch, peaks, ceiling, steps=20):
 
     for k in range(3):
         r.step(k)
-    total_ms = r.timed_steps(steps, barrier)
-    kern = r.timed_kernels(steps, barrier)
+    probe_ms = r.timed_steps(steps, barrier) / steps
+    n_steps = max(steps, int(min_seconds * 1e3 / probe_ms))
+    total_ms = r.timed_steps(n_steps, barrier)
+    kern = r.timed_kernels(max(steps, 20), barrier)
+    added, added_b2b = r.timed_added(added_frames_fit(cfg, 24), barrier)
     k_ms = statistics.mean(kern)
-    ms = total_ms / steps
-    out = {"workload": name, "n_inputs": cfg.n_inputs, "n_freq": cfg.n_freq, "t_per_frame": cfg.n_time, "steps": steps,
+    ms = total_ms / n_steps
+    out = {"workload": name, "n_inputs": cfg.n_inputs, "n_freq": cfg.n_freq, "t_per_frame": cfg.n_time, "steps": n_steps,
            "ms_per_step": ms, "value_gbps": 8.0 * cfg.frame_bytes / (ms * 1e-3) / 1e9, "cmac_per_s": cfg.cmacs_per_frame / (ms * 1e-3),
-           "kernel_ms": k_ms, "kernel_ms_min": min(kern), "roofline": tensor_roofline(cfg, k_ms, peaks, ceiling)}
+           "kernel_ms": k_ms, "kernel_ms_min": min(kern), "kernel_ms_median": statistics.median(kern),
+           "added_frame_kernel_ms": kstats(added), "added_frame_back_to_back_ms": added_b2b,
+           "added_over_first_median": statistics.median(added) / statistics.median(kern),
+           "roofline": tensor_roofline(cfg, k_ms, peaks, ceiling, "sustained")}
+    if cpu:
+        try:
+            c = oracle_sample(cfg)
+            out["cpu_oracle"] = {k: c[k] for k in ("value", "unit", "cores", "sample", "cmac_per_s")}
+        except Exception as e:
+            out["cpu_oracle"] = {"error": str(e)[:160]}
     if cfg.n_frames > 1:
-        # frames ADDED to a running integration (the streamed case: no read between frames), device resident
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        r.x.read(r.out_dev, r.st)
-        barrier()
-        e0.record(r.st)
-        for k in range(steps):
-            r.x.process(r.dev_frames[k % 2], r.st)
-        e1.record(r.st)
-        barrier()
-        r.x.read(r.out_dev, r.st)
-        out["added_frame_kernel_ms"] = e0.elapsed_time(e1) / steps
         # BASELINE.json configs[2]: n_frames consecutive frames from pinned host memory, double-buffered H2D overlapped with
         # the correlation, ONE read at the end
         # (BASELINE.json configs[2]: 64 consecutive seeded frames; a pool of C3_POOL distinct seeded frames is cycled, as
@@ -414,7 +492,10 @@ def main():
     ap.add_argument("--no-sustained", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true")
     ap.add_argument("--sustained-seconds", type=float, default=2.0)
+    ap.add_argument("--oracle-sample", default=None, help=argparse.SUPPRESS)   # child of oracle_one_core: NAME:channels:samples
     args = ap.parse_args()
+    if args.oracle_sample:
+        return oracle_sample_cli(args.oracle_sample)
     cfg = wl.CONFIGS[args.config]
     if args.impl == "reference":
         return run_reference(args, cfg)
@@ -450,25 +531,19 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # ---- leg 1, "burst": W warm-up steps on a cool part, then K whole steps and K per-kernel timings.  A B200 runs this kernel
+    # at 1965 MHz for a few ms before the power cap (1 kW) pulls the clock down, so this leg flatters; it is reported as `burst`
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.15)            # (the sampler's first reading; before the warm-up so that nothing idles between it and the timed steps)
     for k in range(warm):
         r.step(k)
     barrier()
-    # -- timed region 1: K whole steps, CUDA events on the launching stream
-    launches0 = x.kernel_launches
-    total_ms = r.timed_steps(steps, barrier)
-    launches = x.kernel_launches - launches0
-    # -- timed region 2 (same loop, per-kernel events): duration of the dominant kernel (xengine_kernel = xcorr_process)
-    kern_ms = r.timed_kernels(steps, barrier)
-    clocks = sampler.stop()
-
-    total_ms = replicas.max_over_ranks(total_ms, dist, "cuda")
-    ms_per_step = total_ms / steps
+    burst_total = replicas.max_over_ranks(r.timed_steps(steps, barrier), dist, "cuda")
+    burst_kern = r.timed_kernels(max(steps, 20), barrier)
+    burst_clocks = sampler.stop()
+    burst_ms = burst_total / steps
     bits_per_frame = 8.0 * cfg.frame_bytes
-    value = world * bits_per_frame / (ms_per_step * 1e-3) / 1e9
-    cmac_per_s = world * cfg.cmacs_per_frame / (ms_per_step * 1e-3)
 
     # ---- the int8 tensor issue ceiling of this box (resident operands, no TMA / unpack / epilogue): burst and >= 4 s sustained
     ceiling = None
@@ -479,15 +554,54 @@ def main():
             ceiling = None
             probe_error = str(e)[:160]
 
-    # ---- roofline of the dominant kernel (tensor-bound: a dense int8 contraction)
+    # ---- leg 2, power-steady: the same step back to back for >= sustained_seconds (clocks sampled from here on), and straight
+    # behind it, with nothing idling in between, THE timed region of the line: exactly K steps, then the per-kernel timings and
+    # the added-frame launches.  `value`, `ms_per_step` and `roofline` come from this leg.
+    sustained = None
+    warm_total = warm
+    if not args.no_sustained:
+        n_sus = max(steps, int(args.sustained_seconds * 1e3 / burst_ms))
+        warm_total += n_sus // 4 + n_sus
+        clk = ClockSampler(local)
+        clk.start()
+        for k in range(n_sus // 4):                       # bring the part to its steady state first (not timed)
+            r.step(k)
+        barrier()
+        sus_total = replicas.max_over_ranks(r.timed_steps(n_sus, barrier), dist, "cuda")
+    else:
+        clk = ClockSampler(local)
+        clk.start()
+    launches0 = x.kernel_launches
+    total_ms = r.timed_steps(steps, barrier)
+    launches = x.kernel_launches - launches0
+    kern_ms = r.timed_kernels(max(steps, 20), barrier)
+    added_ms, added_b2b = r.timed_added(added_frames_fit(cfg, max(24, min(steps, 200))), barrier)
+    clocks = clk.stop()
+    leg = "burst" if args.no_sustained else "sustained"
+    clocks["note"] = ("sampled over the power-steady leg (>= %.1f s of back-to-back steps) and the K timed steps that follow it directly"
+                      % args.sustained_seconds) if leg == "sustained" else "sampled over the K timed steps only (--no-sustained)"
+
+    total_ms = replicas.max_over_ranks(total_ms, dist, "cuda")
+    ms_per_step = total_ms / steps
+    value = world * bits_per_frame / (ms_per_step * 1e-3) / 1e9
+    cmac_per_s = world * cfg.cmacs_per_frame / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (tensor-bound: a dense int8 contraction) against the measured int8 issue ceiling
     k_ms = statistics.mean(kern_ms)
-    # `frac` keeps the 2 x measured bf16 burst peak as denominator (int8:bf16 nominal ratio 4.5:2.25) for continuity; the
-    # measured issue ceiling of the int8 pipe itself is beside it (int8_issue_ceiling_tops, frac_*_of_issue_ceiling)
-    roofline = tensor_roofline(cfg, k_ms, peaks, ceiling)
+    roofline = tensor_roofline(cfg, k_ms, peaks, ceiling, leg)
+    roofline["kernel_ms_median"] = statistics.median(kern_ms)
     roofline["kernel_ms_min"] = min(kern_ms)
-    roofline["peak_source"] = f"2 x bf16_tflops (burst) of MEASURED_PEAKS.json [{peaks['source']}]; int8:bf16 nominal ratio 4.5:2.25"
-    roofline["note"] = ("frac may exceed 1: the peak is another dtype's MEASURED library GEMM rate (cuBLAS bf16) x the nominal int8:bf16 ratio, "
-                        "which understates the int8 pipe; frac_useful_of_issue_ceiling is against the measured issue rate of the int8 pipe itself")
+    roofline["kernel_launches_timed"] = len(kern_ms)
+    # frames ADDED to a running integration: what the telescope runs 99.6 % of the time (PAPER.md:99, 10 s cadence)
+    roofline["added_frame_kernel_ms"] = kstats(added_ms)
+    roofline["added_frame_back_to_back_ms"] = added_b2b
+    roofline["added_over_first_median"] = statistics.median(added_ms) / statistics.median(kern_ms)
+    bk = statistics.mean(burst_kern)
+    rb = tensor_roofline(cfg, bk, peaks, ceiling, "burst")
+    roofline["burst"] = {"kernel_ms": kstats(burst_kern), "ms_per_step": burst_ms, "value": world * bits_per_frame / (burst_ms * 1e-3) / 1e9,
+                         "achieved": rb["achieved"], "peak": rb["peak"], "frac": rb["frac"], "frac_of_nominal_4500": rb["frac_of_nominal_4500"],
+                         "frac_of_2x_bf16": rb["frac_of_2x_bf16"], "clocks": burst_clocks,
+                         "note": "K steps from a cool part after W = %d warm-up steps: the first milliseconds before the power cap acts" % warm}
     if ceiling:
         roofline["int8_issue_ceiling"] = ceiling
     elif rank == 0 and not args.no_int8_probe:
@@ -509,37 +623,26 @@ def main():
                     best = g0.elapsed_time(g1) if best is None else min(best, g0.elapsed_time(g1))
             roofline["cublas_int8_gemm_8192_tops_burst"] = 2.0 * 8192 ** 3 / (best * 1e-3) / 1e12
             del ga, gb
-        except Exception as e:  # the probe is context only
+        except Exception as e:  # context only
             roofline["cublas_int8_gemm_8192_tops_burst"] = None
             roofline["int8_probe_error"] = str(e)[:120]
 
-    # ---- sustained leg: the same step back to back for >= sustained_seconds, clocks sampled during this leg only
-    sustained = None
     if not args.no_sustained:
-        n_sus = max(steps, int(args.sustained_seconds * 1e3 / ms_per_step))
-        n_ker = max(20, n_sus // 4)
-        for k in range(n_sus // 4):                       # bring the part to its steady state first (not timed)
-            r.step(k)
-        barrier()
-        sus_sampler = ClockSampler(local)
-        sus_sampler.start()
-        sus_total = r.timed_steps(n_sus, barrier)
-        sus_kern = r.timed_kernels(n_ker, barrier)
-        sus_clocks = sus_sampler.stop()
-        sus_total = replicas.max_over_ranks(sus_total, dist, "cuda")
         sus_ms = sus_total / n_sus
-        sus_k = statistics.mean(sus_kern)
-        sus_ach = 8.0 * cfg.cmacs_per_frame / (sus_k * 1e-3) / 1e12
+        step_tops = 8.0 * cfg.cmacs_per_frame / (sus_ms * 1e-3) / 1e12
         sustained = {"steps": n_sus, "seconds": sus_total * 1e-3, "ms_per_step": sus_ms,
                      "value": world * bits_per_frame / (sus_ms * 1e-3) / 1e9, "unit": "Gb/s",
                      "cmac_per_s": world * cfg.cmacs_per_frame / (sus_ms * 1e-3),
-                     "kernel_ms": sus_k, "kernel_steps": n_ker, "useful_int8_tops": sus_ach,
-                     "frac_of_2x_bf16_sustained": sus_ach / (2.0 * peaks["bf16_sustained"]) if peaks.get("bf16_sustained") else None,
-                     "frac_of_2x_bf16_burst": sus_ach / (2.0 * peaks["bf16_burst"]),
-                     "frac_of_nominal_4500": sus_ach / NOMINAL_INT8_TOPS,
-                     "step_pct_of_nominal_4500": 100.0 * 8.0 * cfg.cmacs_per_frame / (sus_ms * 1e-3) / (NOMINAL_INT8_TOPS * 1e12),
-                     "frac_useful_of_issue_ceiling_sustained": (sus_ach / ceiling["sustained_tops"]) if ceiling else None,
-                     "clocks": sus_clocks}
+                     "step_frac_of_peak": step_tops / roofline["peak"], "step_frac_of_nominal_4500": step_tops / NOMINAL_INT8_TOPS,
+                     "note": "the long leg in front of the K timed steps; kernel times of this state are roofline.kernel_ms*"}
+        # the driver keeps `roofline`: the long leg's figures go there too
+        roofline["sustained_ms_per_step"] = sus_ms
+        roofline["sustained_seconds"] = sus_total * 1e-3
+        roofline["sustained_kernel_ms"] = k_ms
+        roofline["sustained_frac"] = roofline["frac"]
+        roofline["sustained_frac_of_nominal"] = roofline["frac_of_nominal_4500"]
+        roofline["sustained_step_frac_of_peak"] = step_tops / roofline["peak"]
+        roofline["sustained_clocks"] = clocks
 
     # ---- e2e: streamed C-ABI path, HOST frames in, HOST visibilities out, every step
     e2e = None
@@ -616,20 +719,35 @@ def main():
     if solo and not args.no_cpu_baseline:
         cpu = oracle_sample(cfg)
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "cmac_per_s")}
+        cpu["one_core"] = oracle_one_core(cfg)
+
+    if other:
+        # compact copy inside `roofline` (the key the driver's record keeps)
+        roofline["configs"] = {
+            nm: ({"kernel_ms": o["kernel_ms"], "kernel_ms_median": o["kernel_ms_median"], "kernel_ms_min": o["kernel_ms_min"],
+                  "ms_per_step": o["ms_per_step"], "frac": o["roofline"]["frac"], "frac_of_nominal": o["roofline"]["frac_of_nominal_4500"],
+                  "added_frame_kernel_ms_median": o["added_frame_kernel_ms"]["median"],
+                  "added_frame_kernel_ms_min": o["added_frame_kernel_ms"]["min"], "added_over_first_median": o["added_over_first_median"],
+                  "streamed_gbps": (o.get("streamed") or {}).get("value"), "h2d_only_gbps": (o.get("streamed") or {}).get("h2d_only_gbps")}
+                 if "error" not in o else o)
+            for nm, o in other.items()}
 
     if rank == 0:
         peak = roofline["peak"]
         line = {
-            "metric": "xengine_input_gbps", "value": value, "unit": "Gb/s", "n_gpus": world, "steps": steps, "warmup": warm,
+            "metric": "xengine_input_gbps", "value": value, "unit": "Gb/s", "n_gpus": world, "steps": steps, "warmup": warm_total,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8",
             "data": "synthetic",
             "config": {"workload": cfg.name, "n_inputs": cfg.n_inputs, "n_freq": cfg.n_freq, "t_per_frame": cfg.n_time,
                        "frame_bytes": cfg.frame_bytes, "step": "xcorr_process + xcorr_read (one integration per frame)", "options": "xcorr_promise_complete_frames(1)",
                        "l2": f"inputs larger than L2: {n_distinct} distinct {cfg.frame_bytes >> 20} MiB frames alternate",
-                       "parallelism": "replicas only" if world > 1 else "1 GPU", "note": cfg.note},
+                       "parallelism": "replicas only" if world > 1 else "1 GPU", "note": cfg.note,
+                       "timed_region": ("exactly K steps directly behind a power-steady leg of >= %.1f s of the same steps (counted in `warmup`); "
+                                        "the K steps from a cool part are roofline.burst" % args.sustained_seconds) if leg == "sustained"
+                                       else "K steps after W warm-up steps (--no-sustained)"},
             "cmac_per_s": cmac_per_s,
             "pct_int8_peak_nominal": 100.0 * 8.0 * cmac_per_s / world / (NOMINAL_INT8_TOPS * 1e12),
-            "pct_int8_peak_measured": 100.0 * 8.0 * cmac_per_s / world / (peak * 1e12),
+            "pct_int8_issue_ceiling_measured": 100.0 * 8.0 * cmac_per_s / world / (peak * 1e12),
             "paper_context": "51.2 Gb/s per 3-GPU server, 819.2 Gb/s over 16 servers (PAPER.md Table I; other hardware)",
             "roofline": roofline, "sustained": sustained, "cpu_baseline": cpu, "e2e": e2e, "other_configs": other,
             "next_rows": next_rows, "gpu_launches": int(launches), "clocks": clocks,
