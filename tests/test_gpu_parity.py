@@ -427,6 +427,46 @@ def test_c5_full_size_stress(xb):
     x.close()
 
 
+def test_c4_two_distinct_frames_added_full_size(xb):
+    """The telescope's steady state at full size (the kernels "simply add to the output of the last run"): two
+    distinct C4 frames into one integration -- the second takes the added-frame epilogue (bulk reduce-adds) on every tile of
+    the N = 2048 schedule -- against the sum of the oracle's results: whole channels from both schedule regimes, sampled
+    pairs over all channels, the total-power identity on two more channels."""
+    c = wl.CONFIGS["C4"]
+    frames = [c.frame(0), c.frame(1)]
+    assert not np.array_equal(frames[0][:64], frames[1][:64])
+    got = run_gpu(xb, frames, promise=True)
+    chans = [0, 7, 14, 15]
+    want = sum(_channels(fr, chans).astype(np.int64) for fr in frames)
+    assert np.array_equal(got[chans], want)
+    n, f = c.n_inputs, c.n_freq
+    rng = np.random.default_rng(41)
+    idx = _sample_pairs(rng, n, f, 3000, [(0, 0, 0), (f - 1, n - 1, n - 1), (0, 255, 256), (f - 1, 0, n - 1), (5, 1023, 1024)])
+    p = idx[:, 1].astype(np.int64) * (2 * n - idx[:, 1] + 1) // 2 + (idx[:, 2] - idx[:, 1])
+    assert np.array_equal(got[idx[:, 0], p].astype(np.int64), sum(oracle.pairs(fr, idx).astype(np.int64) for fr in frames))
+    for ch in (3, 11):
+        tp = sum(int(oracle.identity_total_power(np.ascontiguousarray(fr[:, ch, :])[:, None, :])[0]) for fr in frames)
+        assert int(oracle.lhs_total_power(got[ch][None], n)[0]) == tp
+
+
+def test_c5_frame_processed_twice_full_size(xb):
+    """C5 (2 GiB frame, 2048 stages per item) processed TWICE into one integration: first-frame epilogue, then the added-frame
+    epilogue on every tile; by linearity the result is exactly 2 x the oracle's -- whole channels from both schedule regimes,
+    the closed form of the constant block on all channels, sampled pairs elsewhere."""
+    c = wl.CONFIGS["C5"]
+    fr = c.frame()
+    got = run_gpu(xb, [fr, fr], promise=True)
+    n, f, t = c.n_inputs, c.n_freq, c.n_time
+    chans = [0, 24, 31]
+    assert np.array_equal(got[chans], 2 * _channels(fr, chans).astype(np.int64))
+    blk = np.concatenate([np.arange(oracle.pair_index(n, i, i), oracle.pair_index(n, i, 255) + 1) for i in range(256)])
+    assert (got[:, blk, 0] == 2 * 128 * t).all() and (got[:, blk, 1] == 0).all()
+    rng = np.random.default_rng(43)
+    idx = _sample_pairs(rng, n, f, 1200, [(0, 255, 256), (f - 1, 0, 511), (7, 300, 300), (f - 1, 511, 511)])
+    p = idx[:, 1].astype(np.int64) * (2 * n - idx[:, 1] + 1) // 2 + (idx[:, 2] - idx[:, 1])
+    assert np.array_equal(got[idx[:, 0], p].astype(np.int64), 2 * oracle.pairs(fr, idx).astype(np.int64))
+
+
 C3_POOL = 4   # distinct seeded 1 GiB frames, cycled 16 times = the 64 consecutive frames of BASELINE.json:configs[2] (SURVEY.md 8(d))
 
 
