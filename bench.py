@@ -200,7 +200,7 @@ def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
         e = [ev() for _ in range(4)]
         with torch.cuda.stream(st):
             e[0].record(st)
-            a.assemble(pk_dev[r % 2], n_pk, 10 ** 12, frame, flags, lost, counts, stream=st, account_into=x)
+            a.assemble(pk_dev[r % 2], n_pk, 10 ** 12, frame, False, lost, counts, stream=st, account_into=x)   # as the streamed path: no flag field
             e[1].record(st)
             x.process(frame, st)
             e[2].record(st)
@@ -211,6 +211,21 @@ def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
     for e in evs[3:]:
         for k, nm in enumerate(names):
             times[nm].append(e[k].elapsed_time(e[k + 1]) * 1e3)
+    # the same fused call with the optional flag field written as well (callers that want to keep it)
+    with_field = []
+    evs = []
+    for r in range(reps + 3):
+        e = [ev() for _ in range(2)]
+        with torch.cuda.stream(st):
+            e[0].record(st)
+            a.assemble(pk_dev[r % 2], n_pk, 10 ** 12, frame, flags, lost, counts, stream=st, account_into=x)
+            e[1].record(st)
+            x.process(frame, st)
+            x.read_normalized(vis, stream=st)
+        evs.append(e)
+    torch.cuda.synchronize()
+    for e in evs[3:]:
+        with_field.append(e[0].elapsed_time(e[1]) * 1e3)
     # the two-call form for callers that bring their own flag field: xcorr_assemble, then xcorr_norm_process_dev on its outputs
     sep = {"assemble": [], "norm_process": []}
     evs = []
@@ -251,16 +266,18 @@ def measure_next_rows(cfg, x, xb, torch, st, host_frame, peaks, reps: int = 20):
     a.close()
     us = {k: statistics.mean(v) for k, v in times.items()}
     us_sep = {k: statistics.mean(v) for k, v in sep.items()}
-    asm_bytes = n_pk * pbytes + cfg.frame_bytes + cfg.frame_bytes // 8
+    asm_bytes = n_pk * pbytes + cfg.frame_bytes          # packets in, frame out (no flag field in the fused form as timed)
     flag_bytes = cfg.frame_bytes // 8
     return {
         "what": "packets (arrival order, device resident) -> xcorr_assemble_accounted (assembly + flag / loss accounting in one pass) -> "
                 "xcorr_process -> xcorr_read_normalized; per-call CUDA-event means over %d repetitions" % reps,
         "packets": n_pk, "packet_bytes": pbytes, "kept_dup_rejected_lostpos": c, "us": us,
-        "us_two_call_form": us_sep,
+        "us_two_call_form": us_sep, "us_two_call_form_total": sum(us_sep.values()),
+        "us_assemble_accounted_with_flag_field": statistics.mean(with_field),
         "assemble_roofline": {"bound": "hbm", "achieved": asm_bytes / (us["assemble_accounted"] * 1e-6) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                               "frac": asm_bytes / (us["assemble_accounted"] * 1e-6) / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": asm_bytes,
-                              "note": "2 kernels in the timed call: packet_claim_kernel + assemble_kernel<true>; the optional flag field is written too here"},
+                              "note": "2 kernels in the timed call: packet_claim_kernel + assemble_kernel<true>, no flag field written (as xcorr_stream_submit_packets "
+                                      "calls it); us_two_call_form_total is what it replaces (xcorr_assemble with the flag field + xcorr_norm_process_dev)"},
         "flag_count_roofline": {"bound": "hbm", "achieved": flag_bytes / (us_sep["norm_process"] * 1e-6) / 1e9, "peak": peaks["hbm_gbs"],
                                 "unit": "GB/s", "frac": flag_bytes / (us_sep["norm_process"] * 1e-6) / 1e9 / peaks["hbm_gbs"],
                                 "algorithmic_bytes": flag_bytes,

@@ -495,7 +495,8 @@ class Assembler:
 
     def assemble(self, packets, n_packets: int, seq0: int, frame=None, flags=None, lost=None, counts=None, stream=None, account_into=None):
         """packets: CUDA or pinned-CPU uint8 tensor holding >= n_packets packets back to back (arrival order).
-        frame / flags / lost / counts: CUDA output tensors (allocated if None).  -> (frame, flags, lost, counts).
+        frame / flags / lost / counts: CUDA output tensors (allocated if None; ``flags=False``: no flag field is written and
+        None is returned in its place).  -> (frame, flags, lost, counts).
         account_into: an ``XCorr`` with normalisation enabled -> xcorr_assemble_accounted (flags and losses are counted into
         that handle in the same pass; no separate norm_process call is needed)."""
         import torch
@@ -505,17 +506,22 @@ class Assembler:
             raise ValueError("host packets must be page-locked (pin_memory) so the GPU can read them")
         t, f, n = self.t_per_frame, self.n_freq, self.n_inputs
         frame = torch.empty((t, f, n), dtype=torch.uint8, device="cuda") if frame is None else frame
-        flags = torch.empty((t, f, n // 8), dtype=torch.uint8, device="cuda") if flags is None else flags
+        if flags is False:           # no flag field wanted (the C ABI's NULL): what the streamed packet path does when it accounts in-pass
+            flags = None
+            fptr = 0
+        else:
+            flags = torch.empty((t, f, n // 8), dtype=torch.uint8, device="cuda") if flags is None else flags
+            fptr = flags.data_ptr()
         lost = torch.empty(f, dtype=torch.int32, device="cuda") if lost is None else lost
         counts = torch.empty(4, dtype=torch.int32, device="cuda") if counts is None else counts
-        if frame.numel() != t * f * n or flags.numel() * 8 != t * f * n or lost.numel() != f or counts.numel() != 4:
+        if frame.numel() != t * f * n or (flags is not None and flags.numel() * 8 != t * f * n) or lost.numel() != f or counts.numel() != 4:
             raise ValueError("output tensor of the wrong size")
         pptr = packets.data_ptr() if packets is not None else 0
         if account_into is None:
-            rc = xcorr_assemble(self.handle, pptr, n_packets, seq0, frame.data_ptr(), flags.data_ptr(), lost.data_ptr(), counts.data_ptr(),
+            rc = xcorr_assemble(self.handle, pptr, n_packets, seq0, frame.data_ptr(), fptr, lost.data_ptr(), counts.data_ptr(),
                                 _stream_handle(stream))
         else:
-            rc = xcorr_assemble_accounted(self.handle, account_into.handle, pptr, n_packets, seq0, frame.data_ptr(), flags.data_ptr(),
+            rc = xcorr_assemble_accounted(self.handle, account_into.handle, pptr, n_packets, seq0, frame.data_ptr(), fptr,
                                           lost.data_ptr(), counts.data_ptr(), account_into._stream(stream))
         if rc != XCORR_OK:
             raise XCorrError(rc, "xcorr_assemble")
