@@ -45,10 +45,11 @@ import numpy as np  # noqa: E402
 import workloads as wl  # noqa: E402
 
 NOMINAL_INT8_TOPS = 4500.0  # dense int8, B200 nominal (2x the 2.25 PFLOP/s dense bf16 figure)
-# dram__bytes_read.sum + dram__bytes_write.sum of xengine_kernel<false> for one C2 launch, from the committed
-# ncu --set full capture summarised in profiles/ (None until a capture exists)
-# profiles/r02_ncu_full_bench_c2.md (268.5 MB read + 9.6 MB written) and r02_ncu_full_bench_c4_c5.md
-NCU_TRAFFIC_BYTES = {"C2": 278.08e6, "C3": None, "C4": 675.4e6, "C5": 4156.4e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE xengine_kernel launch, typed in from the committed ncu --set full captures
+# (cold caches; profiles/r03_ncu_full_added_frames.md for C2 / C3 / C5, profiles/r02_ncu_full_bench_c4_c5.md for C4):
+# first-frame launch (the step the line times) and a launch ADDED to a running integration (reduce-adds into the slots)
+NCU_TRAFFIC_BYTES = {"C2": 277.36e6, "C3": 1465.30e6, "C4": 675.4e6, "C5": 4158.32e6}
+NCU_TRAFFIC_BYTES_ADDED = {"C2": 332.92e6, "C3": 1916.14e6, "C4": None, "C5": 4234.63e6}
 # tcgen05 MMAs (M256 N256 K32, 2 CTAs) xengine_kernel issues per 32-sample K-step of a 256 x 256 super-tile
 MMAS_DIAG, MMAS_OFFDIAG = 2, 4
 
@@ -395,8 +396,8 @@ def added_frames_fit(cfg, n):
     return max(4, min(n, (16777215 // cfg.n_time - 1) // 2))
 
 
-TRAFFIC_SOURCE = {"C2": "profiles/r02_ncu_full_bench_c2.md", "C4": "profiles/r02_ncu_full_bench_c4_c5.md",
-                  "C5": "profiles/r02_ncu_full_bench_c4_c5.md"}
+TRAFFIC_SOURCE = {"C2": "profiles/r03_ncu_full_added_frames.md (captured 2026-11-06)", "C3": "profiles/r03_ncu_full_added_frames.md (captured 2026-11-06)",
+                  "C4": "profiles/r02_ncu_full_bench_c4_c5.md (round 2)", "C5": "profiles/r03_ncu_full_added_frames.md (captured 2026-11-06)"}
 
 
 def tensor_roofline(cfg, k_ms, peaks, ceiling=None, leg="sustained"):
@@ -416,7 +417,8 @@ def tensor_roofline(cfg, k_ms, peaks, ceiling=None, leg="sustained"):
     iou = issued_over_useful(cfg)
     return {"bound": "tensor", "kernel": "xengine_kernel (xcorr_process)", "achieved": achieved, "peak": peak, "unit": "TOP/s",
             "frac": achieved / peak, "leg": leg, "peak_source": source,
-            "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "traffic_source": TRAFFIC_SOURCE.get(cfg.name),
+            "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "traffic_added_frame": NCU_TRAFFIC_BYTES_ADDED.get(cfg.name),
+            "traffic_source": TRAFFIC_SOURCE.get(cfg.name), "frame_bytes": cfg.frame_bytes,
             "kernel_ms": k_ms, "algorithmic_ops_per_launch": alg_ops,
             "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
             "frac_of_2x_bf16": achieved / (2.0 * bf16), "peak_2x_bf16": 2.0 * bf16,
