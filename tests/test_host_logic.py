@@ -55,3 +55,58 @@ def test_bad_arguments():
         xb.xcorr_debug_schedule(24, 1, 64, 74)
     with pytest.raises(xb.XCorrError):
         xb.xcorr_debug_schedule(16, 1, 64, 0)
+
+
+# ------------------------------------------------------------------ bench.py arithmetic (no GPU: the functions are pure)
+def _bench():
+    import importlib
+    return importlib.import_module("bench")
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_bench_issued_over_useful_counts_the_mmas_of_the_schedule(name):
+    """issued / useful int8 ops: 2 MMAs of 2*256*256*32 ops per 32 samples on a diagonal super-tile, 4 above it, against
+    8 ops per complex MAC of the pairs i <= j -- recounted here from the tile grid."""
+    b = _bench()
+    c = wl.CONFIGS[name]
+    nb = -(-c.n_inputs // 256)
+    issued_per_sample = (2 * nb + 4 * nb * (nb - 1) // 2) * (2 * 256 * 256 * 32) / 32
+    useful_per_sample = 8 * c.n_pairs
+    assert b.issued_over_useful(c) == pytest.approx(issued_per_sample / useful_per_sample, rel=1e-12)
+    if c.n_inputs % 256 == 0:
+        # whole super-tiles: a diagonal tile issues 2 * 65536 MACs for its 32896 useful pairs, an off-diagonal one 4 * 65536 for 65536
+        assert 0.99 < b.issued_over_useful(c) <= 1.0
+
+
+def test_bench_tensor_roofline_uses_the_measured_issue_ceiling():
+    b = _bench()
+    c = wl.CONFIGS["C2"]
+    peaks = {"hbm_gbs": 6500.0, "bf16_burst": 1600.0, "bf16_sustained": 1400.0, "source": "test"}
+    ceiling = {"burst_tops": 4400.0, "sustained_tops": 4500.0}
+    k_ms = 0.1
+    ops = 8.0 * c.n_freq * c.n_time * c.n_pairs
+    r = b.tensor_roofline(c, k_ms, peaks, ceiling, "sustained")
+    assert r["algorithmic_ops_per_launch"] == ops and r["achieved"] == pytest.approx(ops / 1e-4 / 1e12)
+    assert r["peak"] == 4500.0 and r["frac"] == pytest.approx(r["achieved"] / 4500.0) and r["frac"] < 1.0
+    assert r["frac_of_2x_bf16"] == pytest.approx(r["achieved"] / 2800.0)
+    assert b.tensor_roofline(c, k_ms, peaks, ceiling, "burst")["peak"] == 4400.0
+    # no probe in the run: the stand-in is 2 x the measured bf16 rate of the same leg, and the line says so
+    r0 = b.tensor_roofline(c, k_ms, peaks, None, "burst")
+    assert r0["peak"] == 3200.0 and "no probe" in r0["peak_source"]
+    assert r["traffic"] >= c.frame_bytes and r["traffic_added_frame"] > r["traffic"] and "profiles/" in r["traffic_source"]
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_bench_added_frame_launches_stay_inside_the_int32_guard(name):
+    """Resident.timed_added enqueues 1 + 2 n frames into one integration: never more samples than xcorr_process accepts."""
+    b = _bench()
+    c = wl.CONFIGS[name]
+    for want in (24, 200, 10 ** 6):
+        n = b.added_frames_fit(c, want)
+        assert 4 <= n <= want and (2 * n + 1) * c.n_time <= 16777215
+
+
+def test_bench_kstats():
+    b = _bench()
+    s = b.kstats([3.0, 1.0, 2.0, 10.0])
+    assert s == {"mean": 4.0, "median": 2.5, "min": 1.0, "launches": 4}
