@@ -46,10 +46,10 @@ import workloads as wl  # noqa: E402
 
 NOMINAL_INT8_TOPS = 4500.0  # dense int8, B200 nominal (2x the 2.25 PFLOP/s dense bf16 figure)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE xengine_kernel launch, typed in from the committed ncu --set full captures
-# (cold caches; profiles/r03_ncu_full_added_frames.md for C2 / C3 / C5, profiles/r02_ncu_full_bench_c4_c5.md for C4):
+# (cold caches; profiles/r03_ncu_full_added_frames.md):
 # first-frame launch (the step the line times) and a launch ADDED to a running integration (reduce-adds into the slots)
-NCU_TRAFFIC_BYTES = {"C2": 277.36e6, "C3": 1465.30e6, "C4": 675.4e6, "C5": 4158.32e6}
-NCU_TRAFFIC_BYTES_ADDED = {"C2": 332.92e6, "C3": 1916.14e6, "C4": None, "C5": 4234.63e6}
+NCU_TRAFFIC_BYTES = {"C2": 277.36e6, "C3": 1465.30e6, "C4": 668.54e6, "C5": 4158.32e6}
+NCU_TRAFFIC_BYTES_ADDED = {"C2": 332.92e6, "C3": 1916.14e6, "C4": 951.01e6, "C5": 4234.63e6}
 # tcgen05 MMAs (M256 N256 K32, 2 CTAs) xengine_kernel issues per 32-sample K-step of a 256 x 256 super-tile
 MMAS_DIAG, MMAS_OFFDIAG = 2, 4
 
@@ -397,7 +397,7 @@ def added_frames_fit(cfg, n):
 
 
 TRAFFIC_SOURCE = {"C2": "profiles/r03_ncu_full_added_frames.md (captured 2026-11-06)", "C3": "profiles/r03_ncu_full_added_frames.md (captured 2026-11-06)",
-                  "C4": "profiles/r02_ncu_full_bench_c4_c5.md (round 2)", "C5": "profiles/r03_ncu_full_added_frames.md (captured 2026-11-06)"}
+                  "C4": "profiles/r03_ncu_full_added_frames.md (captured 2026-11-06)", "C5": "profiles/r03_ncu_full_added_frames.md (captured 2026-11-06)"}
 
 
 def tensor_roofline(cfg, k_ms, peaks, ceiling=None, leg="sustained"):
